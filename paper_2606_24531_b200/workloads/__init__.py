@@ -1,0 +1,106 @@
+"""Seeded synthetic workloads (BASELINE.json ``configs[0..4]``).
+
+The paper measures on real FASTQ NA12878, a repetitive genome, enwik9 and silesia
+(PAPER.md:65-68); none is available, so these generators take their *shapes* and stand in for
+them (recipe in DESIGN.md). This module holds no codec arithmetic and is the only code that the
+oracle side (tests, bench input preparation) and the CUDA side both consume.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from dataclasses import dataclass
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_DIR, "libaceapex_workloads.so")
+_SRC = os.path.join(_DIR, "gen.c")
+_lock = threading.Lock()
+_lib = None
+
+KINDS = {"markov": 0, "fastq": 1, "genome": 2, "text": 3, "random": 4, "mixed": 5}
+SEED_BASE = 0xACEA9E00
+MIB = 1 << 20
+
+
+def build(force: bool = False) -> str:
+    if not force and os.path.exists(_SO) and os.path.getmtime(_SO) >= os.path.getmtime(_SRC):
+        return _SO
+    tmp = _SO + f".tmp{os.getpid()}"
+    subprocess.run(["gcc", "-std=c11", "-O2", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"],
+                   check=True, cwd=_DIR)
+    os.replace(tmp, _SO)
+    return _SO
+
+
+def _get():
+    global _lib
+    with _lock:
+        if _lib is None:
+            L = C.CDLL(build())
+            L.aceapex_workload_generate.argtypes = [C.c_int, C.c_uint64, C.c_void_p, C.c_size_t]
+            L.aceapex_workload_generate.restype = C.c_int
+            _lib = L
+    return _lib
+
+
+def generate(kind: str, nbytes: int, seed: int) -> np.ndarray:
+    """``nbytes`` of profile ``kind`` ('markov', 'fastq', 'genome', 'text', 'random', 'mixed')."""
+    out = np.empty(max(1, nbytes), dtype=np.uint8)
+    rc = _get().aceapex_workload_generate(KINDS[kind], seed & 0xFFFFFFFFFFFFFFFF, out.ctypes.data_as(C.c_void_p), nbytes)
+    if rc != 0:
+        raise ValueError(f"workload generator failed for kind={kind}")
+    return out[:nbytes]
+
+
+@dataclass(frozen=True)
+class Config:
+    """One BASELINE.json config: the data recipe plus the encoder policy it is run with."""
+    name: str
+    kind: str
+    nbytes: int
+    seed: int
+    offset_width: int
+    encoder: dict          # oracle encoder parameters (policy; readings A12, A15)
+    stands_in_for: str
+
+    def data(self, nbytes: int | None = None) -> np.ndarray:
+        return generate(self.kind, self.nbytes if nbytes is None else nbytes, self.seed)
+
+
+# Encoder policies. `literal` is the north_star wording taken literally (accept every match of
+# >= 4 bytes, no scheduling promises); `scheduled` is the policy the large configs run with
+# (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks.
+POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
+POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64)
+
+CONFIGS = {
+    "markov_1m": Config("markov_1m", "markov", 1 * MIB, SEED_BASE + 1, 4, POLICY_LITERAL,
+                        "smoke config (BASELINE.json configs[0])"),
+    "fastq_64m": Config("fastq_64m", "fastq", 64 * MIB, SEED_BASE + 2, 4, POLICY_SCHEDULED,
+                        "clean (real FASTQ NA12878), PAPER.md:65"),
+    "genome_256m": Config("genome_256m", "genome", 256 * MIB, SEED_BASE + 3, 8, POLICY_SCHEDULED,
+                          "repeat (repetitive genome), PAPER.md:66"),
+    "text_256m": Config("text_256m", "text", 256 * MIB, SEED_BASE + 4, 4, POLICY_SCHEDULED,
+                        "enwik9 (English text), PAPER.md:67"),
+    "mixed_1g": Config("mixed_1g", "mixed", 1024 * MIB, SEED_BASE + 5, 4, POLICY_SCHEDULED,
+                       "silesia (mixed), PAPER.md:68"),
+}
+CONFIG_ORDER = ["markov_1m", "fastq_64m", "genome_256m", "text_256m", "mixed_1g"]
+
+
+def seek_ids(n_blocks: int, count: int, seed: int) -> np.ndarray:
+    """``count`` uniformly random block ids (duplicates allowed), seeded (splitmix64)."""
+    ids = np.empty(count, dtype=np.uint64)
+    s = np.uint64(seed & 0xFFFFFFFFFFFFFFFF)
+    with np.errstate(over="ignore"):
+        idx = np.arange(1, count + 1, dtype=np.uint64)
+        z = s + idx * np.uint64(0x9E3779B97F4A7C15)
+        z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+        z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+        z = z ^ (z >> np.uint64(31))
+    ids[:] = z % np.uint64(max(1, n_blocks))
+    return ids

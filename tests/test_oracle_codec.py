@@ -1,0 +1,235 @@
+"""Pins for the oracle codec (FORMAT.md sections 1-5).
+
+What fixes the oracle here: containers assembled by an independent writer (tests/handmade.py)
+whose decoded bytes follow from the plain definition of an absolute-offset copy; round-trip
+identity against the original bytes; agreement of two independent decoders on every block; the
+closed form for N equal bytes; the validator's invariants; the paper's three-phase isolation
+check.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_24531_b200 import workloads as W
+
+from handmade import B, build_container, build_record, container_from_tokens, expand
+
+
+def handmade_case():
+    """3 blocks: doubling matches with length escapes and tags 1..11; a source spanning two blocks;
+    a min-length match; a literal-length escape; a block with no literals at all."""
+    total = 2 * B + 100
+    seqs0 = [(8, 8, 0)] + [(0, 1 << k, 0) for k in range(4, 14)]
+    lits0 = b"ABCDEFGH"
+    lits1 = b"0123456789" + bytes((i * 7 + 3) & 0xFF for i in range(300)) + b"tail" * 4014 + b"xy"
+    seqs1 = [(10, 12, B - 5), (300, 4, 3)]
+    assert 10 + 12 + 300 + 4 + (len(lits1) - 310) == B
+    seqs2 = [(0, 100, B + 10)]
+    lits2 = b""
+    blocks = [(seqs0, lits0), (seqs1, lits1), (seqs2, lits2)]
+    return total, blocks
+
+
+def test_handmade_container_decodes_to_plain_definition():
+    total, blocks = handmade_case()
+    want = expand(total, blocks)
+    assert want[:16] == b"ABCDEFGHABCDEFGH" and want[B - 5:B] == b"DEFGH"
+    assert want[B + 10:B + 22] == b"DEFGH0123456"          # the spanning copy
+    c = container_from_tokens(total, blocks)
+    assert oracle.decode_all(c).tobytes() == want
+    with oracle.Isolated(c) as iso:
+        for b in range(3):
+            blk, hops = iso.decode(b, with_hops=True)
+            assert blk.tobytes() == want[b * B:(b + 1) * B]
+        # last byte of block 0 was produced by the 11th match: 11 hops back to a literal
+        assert iso.decode(0, with_hops=True)[1] == 11
+    ll, ml, src, tags = oracle.decode_tokens(c, 0)
+    assert list(tags) == list(range(1, 12)) and int(ml[-1]) == 8192
+    assert list(oracle.decode_tokens(c, 1)[3]) == [1, 0] and list(oracle.decode_tokens(c, 2)[3]) == [0]
+    rep = oracle.validate(c)
+    assert rep.n_matches_spanning == 1 and rep.max_level_seen == 11 and rep.min_match_seen == 4
+    h, lit, ln, off, ex, tg = oracle.decode_streams(c, 1)
+    assert h.n_seq == 2 and h.n_extras == 1 and int(ex[0]) == 300 and list(ln) == [10, 8, 255, 0]
+    assert h.off_nbytes == 2 and list(off) == [(B - 5) & 255, (B - 5) >> 8, 3, 0]
+
+
+ADVERSARIAL = {
+    "empty": b"",
+    "one": b"x",
+    "three": b"abc",
+    "b_minus_1": bytes((i * 131 + (i >> 5)) & 0xFF for i in range(B - 1)),
+    "b_exact": bytes((i * 29 + (i >> 7)) & 0xFF for i in range(B)),
+    "b_plus_1": bytes((i * 17 + (i >> 3)) & 0xFF for i in range(B + 1)),
+    "all_equal": b"\x00" * (3 * B + 77),
+    "all_distinct_cycle": bytes(range(256)) * 200,
+    "period2": b"ab" * 30000,
+    "period3": b"abc" * 20000,
+    "period5": b"abcde" * 15000,
+    "two_blocks_text": (b"the quick brown fox jumps over the lazy dog. " * 800)[: 2 * B],
+}
+
+
+@pytest.mark.parametrize("name", sorted(ADVERSARIAL))
+@pytest.mark.parametrize("policy", ["literal", "scheduled_small"])
+def test_round_trip_adversarial(name, policy):
+    data = ADVERSARIAL[name]
+    params = dict(min_match=4) if policy == "literal" else dict(min_match=8, max_depth=3, window=2, batch=2, threads=3)
+    c = oracle.encode(data, **params)
+    assert oracle.decode_all(c).tobytes() == data
+    i = oracle.info(c)
+    assert i.total_len == len(data) and i.n_blocks == (len(data) + B - 1) // B
+    assert i.container_bytes == c.size
+    rep = oracle.validate(c)
+    if policy != "literal":
+        assert rep.max_depth_seen <= 3
+    with oracle.Isolated(c) as iso:
+        for b in range(i.n_blocks):
+            assert iso.decode(b).tobytes() == data[b * B:(b + 1) * B]
+
+
+def test_closed_form_equal_bytes_doubling():
+    """N equal bytes, T = 4, unbounded chain: 4 literals then matches of 4, 8, 16, ... from
+    position 0, the last one cut at the block end (newest source that still fits); tags 1, 2, ..."""
+    for n in (4, 7, 8, 9, 100, 4096, B - 3, B):
+        c = oracle.encode(b"\x07" * n, min_match=4, chain_depth=1 << 20)
+        ll, ml, src, tags = oracle.decode_tokens(c, 0)
+        want, want_src, pos = [], [], 4
+        while n - pos >= 4:
+            m = min(pos, n - pos)
+            want.append(m)
+            want_src.append(pos - m)   # newest candidate that reaches the limit: 0 while doubling
+            pos += m
+        assert list(ml) == want and [int(s) for s in src] == want_src
+        assert int(ll[0]) == 4 if want else len(ll) == 0
+        assert list(tags) == list(range(1, len(want) + 1))
+        assert oracle.decode_all(c).tobytes() == b"\x07" * n
+
+
+def test_zero_match_block_is_order0_coding():
+    rng = np.random.default_rng(5)
+    data = rng.choice(np.frombuffer(b"ACGT", np.uint8), size=B, p=[0.4, 0.3, 0.2, 0.1]).tobytes()
+    c, st = oracle.encode(data, return_stats=True, min_match=B)   # threshold never met: literals only
+    assert st.n_seq == 0 and st.n_lit == B
+    h = -sum(p * np.log2(p) for p in (0.4, 0.3, 0.2, 0.1)) * B / 8
+    payload = c.size - oracle.info(c).payload_off
+    assert h * 0.97 <= payload <= h * 1.03 + 32 + 48 + 16 * 8
+    assert oracle.decode_all(c).tobytes() == data
+
+
+def test_uniform_random_ratio_near_one():
+    data = W.generate("random", 8 * B, 99)
+    c = oracle.encode(data, min_match=4)
+    assert 0.93 <= data.size / c.size <= 1.0
+
+
+PROFILE_SAMPLES = [("markov_1m", 1 << 20), ("fastq_64m", 2 << 20), ("genome_256m", 2 << 20),
+                   ("text_256m", 2 << 20), ("mixed_1g", 2 << 20)]
+
+
+@pytest.mark.parametrize("name,nbytes", PROFILE_SAMPLES)
+@pytest.mark.parametrize("policy", ["config", "literal"])
+def test_profiles_round_trip_and_decoders_agree(name, nbytes, policy):
+    cfg = W.CONFIGS[name]
+    data = cfg.data(nbytes)
+    params = dict(cfg.encoder) if policy == "config" else dict(W.POLICY_LITERAL)
+    if params.get("window"):
+        params["window"] = 16           # scaled with the sample so that cross-block matches exist
+        params["batch"] = 8
+    if name == "markov_1m" and policy == "literal":
+        pytest.skip("identical to the config policy")
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=4, **params)
+    full = oracle.decode_all(c)
+    assert np.array_equal(full, data)
+    assert oracle.fnv1a64(full) == oracle.fnv1a64(data)            # PAPER.md:41 FNV check
+    rep = oracle.validate(c)                                         # src+len<=dst, tags, D, R
+    assert rep.n_matches_cross + rep.n_matches_intra + rep.n_matches_spanning == rep.n_seq
+    if params.get("max_depth"):
+        assert rep.max_depth_seen <= params["max_depth"]
+    nb = oracle.info(c).n_blocks
+    with oracle.Isolated(c) as iso:
+        step = 1 if nb <= 64 else 5
+        for b in list(range(0, nb, step)) + [nb - 1]:
+            assert np.array_equal(iso.decode(b), data[b * B:(b + 1) * B]), b
+
+
+def test_encoder_result_independent_of_thread_count():
+    data = W.generate("text", 1 << 20, 1234)
+    a = oracle.encode(data, min_match=8, max_depth=4, window=8, batch=4, threads=1)
+    b = oracle.encode(data, min_match=8, max_depth=4, window=8, batch=4, threads=7)
+    assert np.array_equal(a, b)
+
+
+def test_three_phase_isolation_on_the_oracle():
+    """PAPER.md:49-51 applied to decoder #2: region differs before, equals after, rest untouched."""
+    data = W.generate("fastq", 6 * B, 42)
+    c = oracle.encode(data, min_match=8, max_depth=8, window=2, batch=2)
+    for fill in (0x00, 0xA5):
+        buf = np.full(6 * B, fill, np.uint8)
+        target = 4
+        region = slice(target * B, (target + 1) * B)
+        assert oracle.fnv1a64(buf[region]) != oracle.fnv1a64(data[region])          # phase 1
+        with oracle.Isolated(c) as iso:
+            buf[region] = iso.decode(target)
+        assert oracle.fnv1a64(buf[region]) == oracle.fnv1a64(data[region])          # phase 2
+        mask = np.ones(6 * B, bool); mask[region] = False
+        assert np.all(buf[mask] == fill)                                             # phase 3
+
+
+# ---------------------------------------------------------------- invalid containers
+
+def test_rejects_bad_header_fields():
+    c = oracle.encode(b"hello hello hello hello")
+    for off, val in ((0, ord("X")), (8, 2), (12, 15), (13, 5), (14, 16), (15, 11)):
+        bad = c.copy(); bad[off] = val
+        with pytest.raises(oracle.OracleError):
+            oracle.decode_all(bad)
+    with pytest.raises(oracle.OracleError):
+        oracle.decode_all(c[:40])
+    with pytest.raises(oracle.OracleError):
+        oracle.decode_all(c[:-16])
+
+
+def test_rejects_overlapping_or_forward_match():
+    lits = b"abcdefgh" + b"z" * (B - 16)
+    for src, ml in ((4, 8), (8, 8), (1 << 20, 8)):      # overlaps dst / starts at dst / beyond
+        rec = build_record(0, [(8, ml, src)], lits, tags=[1])
+        c = build_container(B, [rec])
+        with pytest.raises(oracle.OracleError) as e:
+            oracle.decode_all(c)
+        assert e.value.code == -4
+        with pytest.raises(oracle.OracleError):
+            oracle.Isolated(c).decode(0)
+        with pytest.raises(oracle.OracleError):
+            oracle.validate(c)
+
+
+def test_rejects_bad_frequency_sum_and_length_mismatch():
+    total, blocks = handmade_case()
+    good = container_from_tokens(total, blocks)
+    i = oracle.info(good)
+    bad = good.copy()
+    # first u16 frequency of block 0's LIT table: record header 32 B, bitmap 32 B
+    p = i.payload_off + 32 + 32
+    bad[p] ^= 1
+    with pytest.raises(oracle.OracleError):
+        oracle.decode_all(bad)
+    # block whose tokens do not add up to the block length
+    rec = build_record(0, [(8, 8, 0)], b"ABCDEFGH" + b"q" * 10)
+    with pytest.raises(oracle.OracleError):
+        oracle.decode_all(build_container(B, [rec]))
+
+
+def test_validator_flags_wrong_tags_and_broken_promises():
+    total, blocks = handmade_case()
+    recs = [build_record(b * B, s, l) for b, (s, l) in enumerate(blocks)]
+    assert oracle.validate(build_container(total, recs)).n_seq == 14
+    wrong = [build_record(0, blocks[0][0], blocks[0][1], tags=[1] * 11)] + recs[1:]
+    with pytest.raises(oracle.OracleError) as e:
+        oracle.validate(build_container(total, wrong))
+    assert e.value.code == -7
+    with pytest.raises(oracle.OracleError) as e:     # depth promise 3 < actual 11
+        oracle.validate(build_container(total, recs, max_depth=3))
+    assert e.value.code == -7
+    with pytest.raises(oracle.OracleError) as e:     # window promise: block 2 reads block 1
+        oracle.validate(build_container(total, recs, window=2))
+    assert e.value.code == -7
