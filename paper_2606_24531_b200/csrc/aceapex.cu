@@ -1,0 +1,381 @@
+// C-ABI of include/aceapex.h: host-side header parse, scratch layout, launch sequencing.
+// Every step of the decode runs in the kernels of entropy.cuh / match.cuh / seek.cuh; there is
+// no CPU decode path in this library.
+#include "../../include/aceapex.h"
+
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "seek.cuh"
+
+using namespace aceapex;
+
+struct aceapex_ctx {
+    Container cv;
+    aceapex_info info;
+    SlotLayout sl;
+    Scratch sc;
+    bool have_scratch;
+    Control *open_ctl;          // tiny internal allocation used by the open-time scan
+    unsigned long long *h_pending;  // pinned, hop-loop read-back
+    uint32_t epoch, tag;
+    uint64_t launches;
+    int sm_count;
+    int device;
+};
+
+namespace {
+
+inline uint32_t rd32(const uint8_t *p) { return (uint32_t)p[0] | (uint32_t)p[1] << 8 | (uint32_t)p[2] << 16 | (uint32_t)p[3] << 24; }
+inline uint64_t rd64(const uint8_t *p) { return (uint64_t)rd32(p) | (uint64_t)rd32(p + 4) << 32; }
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct ScratchOffsets { size_t ctl, done, mark, slot_of, list, ids, slots, pend, total, zero_bytes; };
+
+ScratchOffsets scratch_offsets(uint64_t n_blocks, const SlotLayout &sl, size_t n_slots, size_t n_targets)
+{
+    ScratchOffsets o;
+    size_t p = 0;
+    o.ctl = p; p += sizeof(Control);
+    o.done = p; p += 4 * (size_t)n_blocks;
+    o.mark = p; p += 4 * (size_t)n_blocks;
+    o.slot_of = p; p += 4 * (size_t)n_blocks;
+    o.zero_bytes = p;                          // everything up to here is zeroed by set_scratch
+    p = align_up(p, 8);
+    o.list = p; p += 8 * n_slots;
+    o.ids = p; p += 8 * (n_targets ? n_targets : 1);
+    p = align_up(p, 256);
+    o.slots = p; p += n_slots * (size_t)sl.stride;
+    p = align_up(p, 256);
+    o.pend = p; p += n_targets * (size_t)kB * 8;
+    o.total = align_up(p, 256);
+    return o;
+}
+
+inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
+{
+    uint64_t rest = c->info.total_len - (b << kBlockLog2);
+    return rest < kB ? (uint32_t)rest : kB;
+}
+
+inline size_t entropy_smem() { return 4 * kEntropyWarpSmemWords * sizeof(uint32_t); }
+inline size_t match_smem(const SlotLayout &sl) { return kB + 15 * (size_t)sl.ms + 64; }
+
+int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
+                   uint32_t count, cudaStream_t st)
+{
+    uint32_t units = 3 * (list ? max_slots : count);
+    uint32_t grid = (units + 3) / 4;
+    uint32_t cap = (uint32_t)c->sm_count * 3;
+    if (grid > cap) grid = cap;
+    if (grid == 0) return ACEAPEX_OK;
+    k_entropy<<<grid, 128, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
+                                                 c->sc.ctl);
+    c->launches++;
+    return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+int aceapex_version(void) { return 100; }
+
+const char *aceapex_strerror(int code)
+{
+    switch (code) {
+    case ACEAPEX_OK: return "ok";
+    case ACEAPEX_E_ARG: return "bad argument";
+    case ACEAPEX_E_FORMAT: return "bad container header";
+    case ACEAPEX_E_CAPACITY: return "buffer too small";
+    case ACEAPEX_E_CORRUPT: return "corrupt container";
+    case ACEAPEX_E_RANGE: return "block id or coordinate out of range";
+    case ACEAPEX_E_NOMEM: return "out of host memory";
+    case ACEAPEX_E_CUDA: return "CUDA runtime error";
+    case ACEAPEX_E_STATE: return "scratch not set";
+    default: return "unknown error";
+    }
+}
+
+int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, aceapex_ctx **out)
+{
+    if (!d_container || !out) return ACEAPEX_E_ARG;
+    *out = nullptr;
+    if ((uintptr_t)d_container & 15) return ACEAPEX_E_ARG;
+    if (nbytes < kHeaderBytes) return ACEAPEX_E_FORMAT;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return ACEAPEX_E_CUDA;
+    uint8_t h[kHeaderBytes];
+    if (h_header) memcpy(h, h_header, kHeaderBytes);
+    else if (cudaMemcpy(h, d_container, kHeaderBytes, cudaMemcpyDeviceToHost) != cudaSuccess) return ACEAPEX_E_CUDA;
+
+    // FORMAT.md section 1
+    if (memcmp(h, "ACEAPEX1", 8) != 0 || rd32(h + 8) != 1) return ACEAPEX_E_FORMAT;
+    if (h[12] != kBlockLog2 || (h[13] != 4 && h[13] != 8) || h[14] != kLanes || h[15] != kProbBits) return ACEAPEX_E_FORMAT;
+    const uint64_t total_len = rd64(h + 16), n_blocks = rd64(h + 24);
+    const uint32_t D = rd32(h + 32), R = rd32(h + 36), max_level = rd32(h + 40);
+    const uint64_t index_off = rd64(h + 48), payload_off = rd64(h + 56);
+    if (n_blocks != (total_len + kB - 1) / kB || n_blocks > (1ull << 32) - 2) return ACEAPEX_E_FORMAT;
+    if (index_off != kHeaderBytes || max_level > 15) return ACEAPEX_E_FORMAT;
+    const uint64_t index_bytes = (n_blocks + 1) * 8 + n_blocks * 3 * kLanes * 4;
+    if (payload_off != ((kHeaderBytes + index_bytes + 15) & ~15ull) || payload_off > nbytes) return ACEAPEX_E_FORMAT;
+
+    aceapex_ctx *c = new (std::nothrow) aceapex_ctx();
+    if (!c) return ACEAPEX_E_NOMEM;
+    memset(c, 0, sizeof *c);
+    c->device = dev;
+    const uint8_t *base = static_cast<const uint8_t *>(d_container);
+    c->cv.base = base;
+    c->cv.rec_off = reinterpret_cast<const uint64_t *>(base + kHeaderBytes);
+    c->cv.states = reinterpret_cast<const uint32_t *>(base + kHeaderBytes + (n_blocks + 1) * 8);
+    c->cv.payload = base + payload_off;
+    c->cv.total_len = total_len;
+    c->cv.n_blocks = n_blocks;
+    c->cv.W = h[13]; c->cv.D = D; c->cv.R = R; c->cv.max_level = max_level;
+    c->epoch = 0; c->tag = 0;
+
+    int rc = ACEAPEX_OK;
+    uint64_t edge[2] = { 0, 0 };   // rec_off[0], rec_off[n_blocks]
+    if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK && cudaMemcpy(&edge[0], c->cv.rec_off, 8, cudaMemcpyDeviceToHost) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK && cudaMemcpy(&edge[1], c->cv.rec_off + n_blocks, 8, cudaMemcpyDeviceToHost) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK && (edge[0] != 0 || payload_off + edge[1] > nbytes)) rc = ACEAPEX_E_FORMAT;
+    c->cv.payload_bytes = edge[1];
+
+    if (rc == ACEAPEX_OK && cudaMalloc(&c->open_ctl, sizeof(Control)) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK && cudaMallocHost(&c->h_pending, 64) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK) {
+        Control init;
+        memset(&init, 0, sizeof init);
+        init.first_bad = ~0ull;
+        if (cudaMemcpy(c->open_ctl, &init, sizeof init, cudaMemcpyHostToDevice) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    }
+    if (rc == ACEAPEX_OK && n_blocks) {
+        // one pass over all record headers (one entropy entry point per block)
+        const uint32_t grid = (uint32_t)((n_blocks + 255) / 256);
+        k_scan_records<<<grid, 256>>>(c->cv, c->open_ctl);
+        c->launches++;
+        if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    }
+    Control res;
+    memset(&res, 0, sizeof res);
+    if (rc == ACEAPEX_OK && cudaMemcpy(&res, c->open_ctl, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+    if (rc == ACEAPEX_OK && res.status) rc = ACEAPEX_E_CORRUPT;
+    if (rc == ACEAPEX_OK) {
+        if (cudaFuncSetAttribute(k_entropy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)entropy_smem()) != cudaSuccess)
+            rc = ACEAPEX_E_CUDA;
+    }
+    if (rc != ACEAPEX_OK) { aceapex_close(c); return rc; }
+
+    c->sl = make_slot_layout(res.max_n_seq, c->cv.W);
+    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem(c->sl)) != cudaSuccess) {
+        aceapex_close(c);
+        return ACEAPEX_E_CUDA;
+    }
+    c->info.total_len = total_len;
+    c->info.n_blocks = n_blocks;
+    c->info.container_bytes = payload_off + edge[1];
+    c->info.block_size = kB;
+    c->info.offset_width = c->cv.W;
+    c->info.max_depth = D;
+    c->info.window = R;
+    c->info.max_level = max_level;
+    c->info.max_n_seq = res.max_n_seq;
+    *out = c;
+    return ACEAPEX_OK;
+}
+
+void aceapex_close(aceapex_ctx *c)
+{
+    if (!c) return;
+    if (c->open_ctl) cudaFree(c->open_ctl);
+    if (c->h_pending) cudaFreeHost(c->h_pending);
+    delete c;
+}
+
+int aceapex_info_get(const aceapex_ctx *c, aceapex_info *out)
+{
+    if (!c || !out) return ACEAPEX_E_ARG;
+    *out = c->info;
+    return ACEAPEX_OK;
+}
+
+size_t aceapex_scratch_bytes(const aceapex_ctx *c, size_t n_slots, size_t n_targets)
+{
+    if (!c || n_slots == 0) return 0;
+    return scratch_offsets(c->cv.n_blocks, c->sl, n_slots, n_targets).total;
+}
+
+int aceapex_set_scratch(aceapex_ctx *c, void *d_scratch, size_t nbytes, size_t n_slots, size_t n_targets,
+                        void *cuda_stream)
+{
+    if (!c || !d_scratch || n_slots == 0 || n_slots > 0xFFFFFFFFull / 3 || n_targets > (1u << 18)) return ACEAPEX_E_ARG;
+    if ((uintptr_t)d_scratch & 255) return ACEAPEX_E_ARG;
+    const ScratchOffsets o = scratch_offsets(c->cv.n_blocks, c->sl, n_slots, n_targets);
+    if (nbytes < o.total) return ACEAPEX_E_CAPACITY;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    uint8_t *p = static_cast<uint8_t *>(d_scratch);
+    c->sc.ctl = reinterpret_cast<Control *>(p + o.ctl);
+    c->sc.done = reinterpret_cast<uint32_t *>(p + o.done);
+    c->sc.mark = reinterpret_cast<uint32_t *>(p + o.mark);
+    c->sc.slot_of = reinterpret_cast<uint32_t *>(p + o.slot_of);
+    c->sc.list = reinterpret_cast<uint64_t *>(p + o.list);
+    c->sc.ids = reinterpret_cast<uint64_t *>(p + o.ids);
+    c->sc.slots = p + o.slots;
+    c->sc.pend = reinterpret_cast<uint64_t *>(p + o.pend);
+    c->sc.n_slots = n_slots;
+    c->sc.n_targets = n_targets;
+    c->epoch = 0;
+    c->tag = 0;
+    if (cudaMemsetAsync(p, 0, o.zero_bytes, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    if (cudaMemsetAsync(&c->sc.ctl->first_bad, 0xFF, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    c->have_scratch = true;
+    return ACEAPEX_OK;
+}
+
+int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *cuda_stream)
+{
+    if (!c || (!d_out && c->info.total_len)) return ACEAPEX_E_ARG;
+    if (!c->have_scratch) return ACEAPEX_E_STATE;
+    if (out_capacity < c->info.total_len) return ACEAPEX_E_CAPACITY;
+    if (c->cv.n_blocks == 0) return ACEAPEX_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (++c->epoch == 0) {   // epoch wrapped: stale done flags could alias
+        if (cudaMemsetAsync(c->sc.done, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        c->epoch = 1;
+    }
+    if (cudaMemsetAsync(&c->sc.ctl->watermark, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    const uint32_t aligned = ((uintptr_t)d_out & 15) == 0;
+    for (uint64_t first = 0; first < c->cv.n_blocks; first += c->sc.n_slots) {
+        const uint64_t rest = c->cv.n_blocks - first;
+        const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);
+        int rc = launch_entropy(c, nullptr, nullptr, 0, first, count, st);
+        if (rc != ACEAPEX_OK) return rc;
+        k_match<<<count, kMatchThreads, match_smem(c->sl), st>>>(c->cv, c->sl, c->sc.slots, first, count,
+                                                                static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
+                                                                c->sc.done, c->epoch);
+        c->launches++;
+        if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
+    }
+    return ACEAPEX_OK;
+}
+
+int aceapex_decode_streams(aceapex_ctx *c, uint64_t first, size_t count, void *d_lit, void *d_len, void *d_off,
+                           void *cuda_stream)
+{
+    if (!c || !d_lit || !d_len || !d_off) return ACEAPEX_E_ARG;
+    if (!c->have_scratch) return ACEAPEX_E_STATE;
+    if (count > c->sc.n_slots) return ACEAPEX_E_CAPACITY;
+    if (first + count > c->cv.n_blocks || first + count < first) return ACEAPEX_E_RANGE;
+    if (count == 0) return ACEAPEX_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int rc = launch_entropy(c, nullptr, nullptr, 0, first, (uint32_t)count, st);
+    if (rc != ACEAPEX_OK) return rc;
+    k_export_streams<<<(uint32_t)count, 256, 0, st>>>(c->cv, c->sl, c->sc.slots, first, (uint32_t)count,
+                                                      static_cast<uint8_t *>(d_lit), static_cast<uint8_t *>(d_len),
+                                                      static_cast<uint8_t *>(d_off));
+    c->launches++;
+    return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
+}
+
+int aceapex_decode_blocks(aceapex_ctx *c, const uint64_t *h_ids, size_t n_ids, void *d_out, size_t out_capacity,
+                          uint32_t flags, void *cuda_stream)
+{
+    if (!c || (n_ids && (!h_ids || !d_out)) || flags > ACEAPEX_ABSOLUTE) return ACEAPEX_E_ARG;
+    if (n_ids == 0) return ACEAPEX_OK;
+    if (!c->have_scratch || c->sc.n_targets == 0) return ACEAPEX_E_STATE;
+    const bool absolute = flags == ACEAPEX_ABSOLUTE;
+    size_t need = 0;
+    for (size_t i = 0; i < n_ids; i++) {
+        if (h_ids[i] >= c->cv.n_blocks) return ACEAPEX_E_RANGE;
+        const size_t end = ((absolute ? (size_t)h_ids[i] : i) << kBlockLog2) + block_len_host(c, h_ids[i]);
+        if (end > need) need = end;
+    }
+    if (out_capacity < need) return ACEAPEX_E_CAPACITY;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Control *ctl = c->sc.ctl;
+    const uint32_t S = (uint32_t)(c->sc.n_slots > 0xFFFFFFFFull / 4 ? 0xFFFFFFFFull / 4 : c->sc.n_slots);
+
+    for (size_t base = 0; base < n_ids; base += c->sc.n_targets) {
+        const uint32_t nt = (uint32_t)(n_ids - base < c->sc.n_targets ? n_ids - base : c->sc.n_targets);
+        const uint64_t n_bytes = (uint64_t)nt * kB;
+        if (cudaMemcpyAsync(c->sc.ids, h_ids + base, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess)
+            return ACEAPEX_E_CUDA;
+        k_seek_init<<<(uint32_t)((n_bytes + 255) / 256), 256, 0, st>>>(c->cv, c->sc.ids, nt, c->sc.pend);
+        c->launches++;
+        // With a depth promise D and a slot for every block a hop can touch, D+1 hops always
+        // suffice (hop 0 resolves the target's own literals): enqueue them without reading back.
+        const uint64_t touch = n_bytes < c->cv.n_blocks ? n_bytes : c->cv.n_blocks;
+        const bool fixed = c->cv.D > 0 && (uint64_t)S >= touch;
+        const uint32_t chunks = (uint32_t)((n_bytes + kChunk - 1) / kChunk);
+        const uint32_t cgrid = (chunks + 127) / 128;
+        for (uint32_t hop = 0;; hop++) {
+            if (++c->tag == 0) {
+                if (cudaMemsetAsync(c->sc.mark, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+                c->tag = 1;
+            }
+            if (cudaMemsetAsync(&ctl->n_list, 0, 4, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+            if (cudaMemsetAsync(&ctl->pending, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+            k_seek_collect<<<cgrid, 128, 0, st>>>(c->sc.pend, n_bytes, c->sc.mark, c->sc.slot_of, c->sc.list, ctl,
+                                                  c->tag, S);
+            c->launches++;
+            int rc = launch_entropy(c, c->sc.list, &ctl->n_list, S, 0, 0, st);
+            if (rc != ACEAPEX_OK) return rc;
+            uint32_t pgrid = S < (uint32_t)c->sm_count * 8 ? S : (uint32_t)c->sm_count * 8;
+            k_parse<<<pgrid, kMatchThreads, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.list, &ctl->n_list, S, ctl);
+            c->launches++;
+            k_seek_resolve<<<cgrid, 128, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.pend, nt, c->sc.ids, c->sc.mark,
+                                                  c->sc.slot_of, ctl, c->tag, S, static_cast<uint8_t *>(d_out),
+                                                  (uint64_t)base, absolute ? 1u : 0u);
+            c->launches++;
+            if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
+            if (fixed) {
+                if (hop >= c->cv.D) {
+                    k_seek_check<<<1, 1, 0, st>>>(ctl);
+                    c->launches++;
+                    break;
+                }
+            } else {
+                if (cudaMemcpyAsync(c->h_pending, &ctl->pending, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+                    return ACEAPEX_E_CUDA;
+                if (cudaStreamSynchronize(st) != cudaSuccess) return ACEAPEX_E_CUDA;
+                if (*c->h_pending == 0) break;
+            }
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
+}
+
+int aceapex_seek(aceapex_ctx *c, uint64_t coord, void *d_dst, size_t dst_capacity, uint64_t *block_start_out,
+                 uint32_t *block_len_out, void *cuda_stream)
+{
+    if (!c || !d_dst) return ACEAPEX_E_ARG;
+    if (coord >= c->info.total_len) return ACEAPEX_E_RANGE;
+    const uint64_t b = coord >> kBlockLog2;          // the single coordinate
+    const uint32_t len = block_len_host(c, b);
+    if (dst_capacity < len) return ACEAPEX_E_CAPACITY;
+    if (block_start_out) *block_start_out = b << kBlockLog2;
+    if (block_len_out) *block_len_out = len;
+    return aceapex_decode_blocks(c, &b, 1, d_dst, dst_capacity, ACEAPEX_PACKED, cuda_stream);
+}
+
+int aceapex_device_status(aceapex_ctx *c, void *cuda_stream, uint64_t *first_bad_block, int clear)
+{
+    if (!c) return ACEAPEX_E_ARG;
+    if (!c->have_scratch) return ACEAPEX_E_STATE;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Control h;
+    if (cudaMemcpyAsync(&h, c->sc.ctl, sizeof h, cudaMemcpyDeviceToHost, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    if (first_bad_block) *first_bad_block = h.first_bad;
+    if (clear && h.status) {
+        if (cudaMemsetAsync(&c->sc.ctl->status, 0, 4, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        if (cudaMemsetAsync(&c->sc.ctl->first_bad, 0xFF, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    }
+    return h.status ? ACEAPEX_E_CORRUPT : ACEAPEX_OK;
+}
+
+uint64_t aceapex_launch_count(const aceapex_ctx *c) { return c ? c->launches : 0; }
+
+}  // extern "C"
