@@ -1,0 +1,335 @@
+"""Parity of the CUDA path against the CPU oracle (-m gpu), through the C-ABI.
+
+Bar: bit-exact. Every byte of decode_all against oracle decoder #1; every isolated block against
+oracle decoder #2; the entropy layer on its own against the oracle's per-stream decode
+(PAPER.md:41 checks the ANS round trip separately); the paper's three-phase isolation check
+ with the untouched check extended to the whole buffer and a non-zero fill
+("empty-buffer trap"). Inputs are seeded and synthetic (DESIGN.md recipe).
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_24531_b200 import workloads as W
+
+from handmade import B, build_container, build_record, container_from_tokens
+from test_oracle_codec import ADVERSARIAL, handmade_case
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device; the product has no CPU fallback")
+    from paper_2606_24531_b200 import binding as b
+    return b
+
+
+def dev_out(n, fill=0xA5):
+    return torch.full((max(1, n),), fill, dtype=torch.uint8, device="cuda")
+
+
+def full_check(binding, c, want, n_slots=None, n_targets=16, seek_blocks=None, fills=(0xA5,)):
+    """decode_all == want; listed (default: all) blocks decode in isolation to want's ranges."""
+    want = np.frombuffer(want, np.uint8) if isinstance(want, (bytes, bytearray)) else want
+    n = want.size
+    with binding.Decoder(c, n_slots=n_slots, n_targets=n_targets) as dec:
+        assert dec.info.total_len == n
+        for fill in fills:
+            out = dev_out(n + 64, fill)
+            dec.decode_all(out)
+            dec.check()
+            got = out.cpu().numpy()
+            assert np.array_equal(got[:n], want)
+            assert np.all(got[n:] == fill)                       # nothing beyond total_len
+        nb = int(dec.info.n_blocks)
+        ids = list(range(nb)) if seek_blocks is None else list(seek_blocks)
+        if ids:
+            got = dec.decode_blocks(np.array(ids, np.uint64), dev_out(len(ids) * B)).cpu().numpy()
+            dec.check()
+            for i, b in enumerate(ids):
+                blen = min(B, n - b * B)
+                assert np.array_equal(got[i * B:i * B + blen], want[b * B:b * B + blen]), b
+                assert np.all(got[i * B + blen:(i + 1) * B] == 0xA5)
+        return dec.launch_count
+
+
+# ------------------------------------------------------------------ configs (BASELINE.json configs[0..4])
+
+def test_config0_markov_1m_decode_all_and_seek_every_block(binding):
+    cfg = W.CONFIGS["markov_1m"]
+    data = cfg.data()
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=4, **cfg.encoder)
+    want = oracle.decode_all(c)
+    assert np.array_equal(want, data)
+    assert oracle.info(c).max_depth == 0                         # literal policy: no depth promise -> read-back hop loop
+    full_check(binding, c, want, fills=(0x00, 0xA5))
+    # every block through aceapex_seek, compared with oracle decoder #2
+    with binding.Decoder(c, n_targets=1) as dec, oracle.Isolated(c) as iso:
+        for b in range(int(dec.info.n_blocks)):
+            blk, start, blen = dec.seek(b * B + (b * 37) % B)
+            assert (start, blen) == (b * B, B)
+            assert np.array_equal(blk.cpu().numpy()[:blen], iso.decode(b)), b
+        dec.check()
+
+
+SAMPLES = [("fastq_64m", 6 << 20), ("genome_256m", 6 << 20), ("text_256m", 6 << 20), ("mixed_1g", 6 << 20)]
+
+
+@pytest.mark.parametrize("name,nbytes", SAMPLES)
+@pytest.mark.parametrize("policy", ["scheduled", "literal"])
+def test_profile_samples_bit_exact(binding, name, nbytes, policy):
+    """Several hundred blocks of each profile, ragged tail, under both encoder policies."""
+    cfg = W.CONFIGS[name]
+    nbytes += 12345                                              # ragged last block
+    data = cfg.data(nbytes)
+    params = dict(cfg.encoder) if policy == "scheduled" else dict(W.POLICY_LITERAL)
+    if params.get("window"):
+        params.update(window=24, batch=8)                        # scaled so that cross-block matches exist
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=8, **params)
+    want = oracle.decode_all(c)
+    nb = oracle.info(c).n_blocks
+    rng = np.random.default_rng(7)
+    ids = sorted(set([0, 1, nb // 2, nb - 2, nb - 1] + [int(x) for x in rng.integers(0, nb, 24)]))
+    full_check(binding, c, want, seek_blocks=ids, n_targets=8)
+    with binding.Decoder(c, n_targets=4) as dec, oracle.Isolated(c) as iso:
+        for b in ids[:6] + ids[-2:]:
+            blk, start, blen = dec.seek(b * B + 1)
+            assert np.array_equal(blk.cpu().numpy()[:blen], iso.decode(b)), b
+        dec.check()
+
+
+def test_bench_config_fastq_64m_full_size(binding):
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py times."""
+    cfg = W.CONFIGS["fastq_64m"]
+    data = cfg.data()
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=8, **cfg.encoder)
+    want = oracle.decode_all(c)
+    assert oracle.fnv1a64(want) == oracle.fnv1a64(data)
+    nb = oracle.info(c).n_blocks
+    ids = [int(x) for x in W.seek_ids(nb, 48, W.SEED_BASE + 0x72)] + [0, nb - 1]
+    full_check(binding, c, want, seek_blocks=ids, n_targets=64)
+
+
+# ------------------------------------------------------------------ entropy layer alone
+
+@pytest.mark.parametrize("name", ["markov_1m", "genome_256m"])
+def test_entropy_layer_streams_match_oracle(binding, name):
+    cfg = W.CONFIGS[name]
+    data = cfg.data(40 * B + 999)
+    params = dict(cfg.encoder)
+    if params.get("window"):
+        params.update(window=4, batch=4)
+    c = oracle.encode(data, offset_width=cfg.offset_width, **params)
+    nb = oracle.info(c).n_blocks
+    with binding.Decoder(c) as dec:
+        lit, ln, off = (t.cpu().numpy() for t in dec.decode_streams(0, nb))
+        dec.check()
+    for b in range(nb):
+        h, olit, olen, ooff, _, _ = oracle.decode_streams(c, b)
+        assert np.array_equal(lit[b * B:b * B + olit.size], olit), b
+        assert np.array_equal(ln[b * 8192:b * 8192 + olen.size], olen), b
+        assert np.array_equal(off[b * 32768:b * 32768 + ooff.size], ooff), b
+
+
+# ------------------------------------------------------------------ handmade and adversarial inputs
+
+def test_handmade_tokens_spanning_source_escapes_deep_tags(binding):
+    total, blocks = handmade_case()
+    c = container_from_tokens(total, blocks)
+    want = oracle.decode_all(c)
+    full_check(binding, c, want, fills=(0x00, 0xA5))
+    c8 = container_from_tokens(total, blocks, off_width=8)
+    full_check(binding, c8, want)
+
+
+@pytest.mark.parametrize("name", sorted(ADVERSARIAL))
+def test_adversarial_sizes(binding, name):
+    data = ADVERSARIAL[name]
+    for params in (dict(min_match=4), dict(min_match=8, max_depth=3, window=2, batch=2)):
+        c = oracle.encode(data, **params)
+        want = oracle.decode_all(c)
+        assert want.tobytes() == data
+        full_check(binding, c, want)
+
+
+def test_max_sequences_per_block(binding):
+    """4095 sequences in one block (the most a 16 KiB block can hold: 4 literals, then 4-byte matches)."""
+    lits = b"wxyz"
+    seqs = [(4, 4, 0)] + [(0, 4, 0) for k in range(1, 4095)]
+    blocks = [(seqs, lits)]
+    c = container_from_tokens(B, blocks)
+    want = oracle.decode_all(c)
+    assert want.tobytes() == b"wxyz" * 4096
+    full_check(binding, c, want)
+    # and 4096 single-literal sequences with 255+ escapes in a second block reading the first
+    seqs2 = [(1, 4, 8 * k) for k in range(2048)] + [(300, 5000, 0)]
+    lits2 = bytes((k * 11) & 0xFF for k in range(2048 + 300)) + b"!" * (B - (2048 * 5 + 300 + 5000))
+    c2 = container_from_tokens(2 * B, [(seqs, lits), (seqs2, lits2)])
+    full_check(binding, c2, oracle.decode_all(c2))
+
+
+def test_small_scratch_batches_and_slot_overflow(binding):
+    """decode_all in batches of 5 slots; isolated decode with 3 slots (several passes per hop)."""
+    data = W.generate("text", 40 * B + 17, 77)
+    for params in (dict(min_match=4), dict(min_match=8, max_depth=4, window=3, batch=3)):
+        c = oracle.encode(data, **params)
+        want = oracle.decode_all(c)
+        full_check(binding, c, want, n_slots=5, n_targets=2, seek_blocks=[40, 39, 17, 17, 3, 0])
+        full_check(binding, c, want, n_slots=3, n_targets=1, seek_blocks=[33, 40])
+
+
+# ------------------------------------------------------------------ isolation
+
+@pytest.mark.parametrize("fill", [0x00, 0xA5])
+def test_three_phase_isolation(binding, fill):
+    data = W.generate("fastq", 24 * B + 100, 42)
+    c = oracle.encode(data, min_match=8, max_depth=8, window=2, batch=2)
+    n = data.size
+    with binding.Decoder(c, n_targets=4) as dec:
+        for target in (0, 7, 23, 24):
+            buf = dev_out(n, fill)
+            lo, hi = target * B, min(n, (target + 1) * B)
+            assert oracle.fnv1a64(buf[lo:hi].cpu().numpy()) != oracle.fnv1a64(data[lo:hi])      # phase 1
+            dec.decode_blocks(np.array([target], np.uint64), buf, flags=binding.ABSOLUTE)
+            dec.check()
+            got = buf.cpu().numpy()
+            assert oracle.fnv1a64(got[lo:hi]) == oracle.fnv1a64(data[lo:hi])                     # phase 2
+            assert np.array_equal(got[lo:hi], data[lo:hi])
+            mask = np.ones(n, bool); mask[lo:hi] = False
+            assert np.all(got[mask] == fill)                                                     # phase 3: whole buffer
+        # aceapex_seek writes only block_len bytes of its destination
+        dst = dev_out(B + 32, fill)
+        _, start, blen = dec.seek(n - 1, dst)
+        assert (start, blen) == (24 * B, 100)
+        got = dst.cpu().numpy()
+        assert np.array_equal(got[:100], data[24 * B:]) and np.all(got[100:] == fill)
+
+
+def test_decode_blocks_absolute_duplicates_and_errors(binding):
+    data = W.generate("genome", 9 * B + 5, 11)
+    c = oracle.encode(data, min_match=8, max_depth=6, window=2, batch=2, offset_width=8)
+    with binding.Decoder(c, n_targets=3) as dec:
+        buf = dev_out(data.size)
+        ids = np.array([9, 2, 2, 5, 9, 0, 2], np.uint64)
+        dec.decode_blocks(ids, buf, flags=binding.ABSOLUTE)
+        dec.check()
+        got = buf.cpu().numpy()
+        for b in range(10):
+            lo, hi = b * B, min(data.size, (b + 1) * B)
+            if b in (0, 2, 5, 9):
+                assert np.array_equal(got[lo:hi], data[lo:hi])
+            else:
+                assert np.all(got[lo:hi] == 0xA5)
+        L = binding.lib()
+        one = np.array([10], np.uint64)
+        assert L.aceapex_decode_blocks(dec._ctx, one.ctypes.data_as(C.c_void_p), 1, buf.data_ptr(), buf.numel(), 0, None) == binding.E_RANGE
+        assert L.aceapex_seek(dec._ctx, data.size, buf.data_ptr(), buf.numel(), None, None, None) == binding.E_RANGE
+        assert L.aceapex_seek(dec._ctx, 0, buf.data_ptr(), 100, None, None, None) == binding.E_CAPACITY
+        assert L.aceapex_decode_all(dec._ctx, buf.data_ptr(), data.size - 1, None) == binding.E_CAPACITY
+        two = np.array([0, 1], np.uint64)
+        assert L.aceapex_decode_blocks(dec._ctx, two.ctypes.data_as(C.c_void_p), 2, buf.data_ptr(), 2 * B - 1, 0, None) == binding.E_CAPACITY
+        assert L.aceapex_decode_blocks(dec._ctx, two.ctypes.data_as(C.c_void_p), 2, buf.data_ptr(), buf.numel(), 7, None) == binding.E_ARG
+
+
+def test_unaligned_output_pointer(binding):
+    data = W.generate("text", 5 * B + 3, 5)
+    c = oracle.encode(data, min_match=4)
+    with binding.Decoder(c) as dec:
+        buf = dev_out(data.size + 16)
+        dec.decode_all(buf[3:])
+        dec.check()
+        got = buf.cpu().numpy()
+        assert np.all(got[:3] == 0xA5) and np.array_equal(got[3:3 + data.size], data)
+        assert np.all(got[3 + data.size:] == 0xA5)
+
+
+# ------------------------------------------------------------------ invalid containers
+
+def open_rc(binding, c):
+    t = torch.from_numpy(np.ascontiguousarray(c)).cuda()
+    ctx = C.c_void_p()
+    rc = binding.lib().aceapex_open(t.data_ptr(), t.numel(), None, C.byref(ctx))
+    if rc == 0:
+        binding.lib().aceapex_close(ctx)
+    return rc
+
+
+def test_rejects_bad_header_fields(binding):
+    c = oracle.encode(b"hello hello hello hello")
+    for off, val in ((0, ord("X")), (8, 2), (12, 15), (13, 5), (14, 16), (15, 11)):
+        bad = c.copy(); bad[off] = val
+        assert open_rc(binding, bad) == binding.E_FORMAT
+    assert open_rc(binding, c[:48].copy()) == binding.E_FORMAT
+    assert open_rc(binding, c[:-16].copy()) == binding.E_FORMAT
+    assert open_rc(binding, c) == 0
+
+
+def expect_corrupt(binding, c, n, bad_block=None):
+    """The device reports CORRUPT, leaves the bad block unwritten and never writes out of bounds."""
+    with binding.Decoder(c, n_targets=2) as dec:
+        out = dev_out(n + 4096)
+        dec.decode_all(out)
+        rc, first = dec.device_status(clear=True)
+        assert rc == binding.E_CORRUPT
+        got = out.cpu().numpy()
+        assert np.all(got[n:] == 0xA5)
+        if bad_block is not None:
+            assert first == bad_block
+            assert np.all(got[bad_block * B:min(n, (bad_block + 1) * B)] == 0xA5)
+        assert dec.device_status()[0] == 0                       # cleared
+        buf = dev_out(B + 64)
+        dec.decode_blocks(np.array([bad_block or 0], np.uint64), buf)
+        assert dec.device_status(clear=True)[0] == binding.E_CORRUPT
+        assert np.all(buf.cpu().numpy()[B:] == 0xA5)
+
+
+def test_rejects_overlapping_or_forward_match(binding):
+    lits = b"abcdefgh" + b"z" * (B - 16)
+    for src, ml in ((4, 8), (8, 8), (1 << 20, 8)):              # overlaps dst / starts at dst / beyond
+        rec = build_record(0, [(8, ml, src)], lits, tags=[1])
+        expect_corrupt(binding, build_container(B, [rec]), B, 0)
+
+
+def test_rejects_bad_frequency_sum_state_and_token_sums(binding):
+    total, blocks = handmade_case()
+    good = container_from_tokens(total, blocks)
+    i = oracle.info(good)
+    bad = good.copy()
+    bad[i.payload_off + 32 + 32] ^= 1                            # block 0 LIT table: sum != 4096
+    expect_corrupt(binding, bad, total, 0)
+    bad = good.copy()
+    st = 64 + (i.n_blocks + 1) * 8 + (1 * 3 + 1) * 32 * 4 + 5 * 4   # block 1, LEN stream, lane 5
+    bad[st] ^= 0x40
+    expect_corrupt(binding, bad, total, 1)
+    rec = build_record(0, [(8, 8, 0)], b"ABCDEFGH" + b"q" * 10)  # tokens do not add up to the block length
+    expect_corrupt(binding, build_container(B, [rec]), B, 0)
+
+
+def test_open_rejects_corrupt_record_header(binding):
+    total, blocks = handmade_case()
+    good = container_from_tokens(total, blocks)
+    i = oracle.info(good)
+    bad = good.copy()
+    bad[i.payload_off + 6] = 9                                   # off_nbytes > W
+    assert open_rc(binding, bad) == binding.E_CORRUPT
+    bad = good.copy()
+    bad[i.payload_off + 8] ^= 0x10                               # n_words[LIT] changed: section layout no longer fits
+    assert open_rc(binding, bad) == binding.E_CORRUPT
+
+
+def test_broken_depth_promise_is_reported_by_isolated_decode(binding):
+    total, blocks = handmade_case()                              # real chase depth 11
+    recs = [build_record(b * B, s, l) for b, (s, l) in enumerate(blocks)]
+    c = build_container(total, recs, max_depth=3)
+    with binding.Decoder(c, n_targets=2) as dec:
+        out = dev_out(total)
+        dec.decode_all(out)                                      # decode_all does not rely on the promise
+        dec.check()
+        assert np.array_equal(out.cpu().numpy(), oracle.decode_all(c))
+        dec.decode_blocks(np.array([0], np.uint64), dev_out(B))
+        assert dec.device_status(clear=True)[0] == binding.E_CORRUPT
