@@ -151,6 +151,17 @@ uint64_t aceapex_launch_count(const aceapex_ctx *ctx);
 int aceapex_decode_streams(aceapex_ctx *ctx, uint64_t first, size_t count, void *d_lit, void *d_len,
                            void *d_off, void *cuda_stream);
 
+/* Per-kernel device timing (measurement support for bench.py). While
+ * enabled, every kernel the library launches is bracketed by two CUDA events on the stream it
+ * is launched on. aceapex_profile_read synchronises the device and returns, for each kernel id
+ * in [0, ACEAPEX_N_KERNELS), the launches and the summed device milliseconds since the last
+ * read (HOST arrays of ACEAPEX_N_KERNELS entries; either may be NULL), then resets the sums. */
+enum { ACEAPEX_N_KERNELS = 16 };
+int aceapex_profile_enable(aceapex_ctx *ctx, int on);
+int aceapex_profile_read(aceapex_ctx *ctx, uint64_t *launches, double *ms);
+/* Name of kernel id `id` (NULL if id is not used). */
+const char *aceapex_kernel_name(int id);
+
 const char *aceapex_strerror(int code);
 
 void aceapex_close(aceapex_ctx *ctx);

@@ -24,7 +24,9 @@ E_ARG, E_FORMAT, E_CAPACITY, E_CORRUPT, E_RANGE, E_NOMEM, E_CUDA, E_STATE = -1, 
 # every symbol include/aceapex.h declares
 SYMBOLS = ["aceapex_version", "aceapex_open", "aceapex_info_get", "aceapex_scratch_bytes", "aceapex_set_scratch",
            "aceapex_decode_all", "aceapex_decode_blocks", "aceapex_seek", "aceapex_device_status",
-           "aceapex_launch_count", "aceapex_decode_streams", "aceapex_strerror", "aceapex_close"]
+           "aceapex_launch_count", "aceapex_decode_streams", "aceapex_profile_enable", "aceapex_profile_read",
+           "aceapex_kernel_name", "aceapex_strerror", "aceapex_close"]
+N_KERNELS = 16
 
 
 class AceapexError(RuntimeError):
@@ -66,6 +68,9 @@ def lib():
             L.aceapex_device_status.argtypes = [vp, vp, C.POINTER(u64), C.c_int]
             L.aceapex_launch_count.argtypes = [vp]; L.aceapex_launch_count.restype = u64
             L.aceapex_decode_streams.argtypes = [vp, u64, sz, vp, vp, vp, vp]
+            L.aceapex_profile_enable.argtypes = [vp, C.c_int]
+            L.aceapex_profile_read.argtypes = [vp, vp, vp]
+            L.aceapex_kernel_name.argtypes = [C.c_int]; L.aceapex_kernel_name.restype = C.c_char_p
             L.aceapex_strerror.argtypes = [C.c_int]; L.aceapex_strerror.restype = C.c_char_p
             L.aceapex_close.argtypes = [vp]; L.aceapex_close.restype = None
             _lib = L
@@ -179,6 +184,22 @@ class Decoder:
         rc, bad = self.device_status(stream=stream)
         if rc != 0:
             raise AceapexError(rc, f"device status (first bad block {bad})")
+
+    # -- aceapex_profile_enable / aceapex_profile_read
+    def profile_enable(self, on: bool = True):
+        _check(lib().aceapex_profile_enable(self._ctx, 1 if on else 0), "aceapex_profile_enable")
+
+    def profile_read(self) -> dict:
+        """{kernel name: (launches, summed device ms)} since the last read; synchronises."""
+        n = (C.c_uint64 * N_KERNELS)()
+        ms = (C.c_double * N_KERNELS)()
+        _check(lib().aceapex_profile_read(self._ctx, n, ms), "aceapex_profile_read")
+        out = {}
+        for i in range(N_KERNELS):
+            name = lib().aceapex_kernel_name(i)
+            if name and n[i]:
+                out[name.decode()] = (int(n[i]), float(ms[i]))
+        return out
 
     @property
     def launch_count(self) -> int:

@@ -6,23 +6,54 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "seek.cuh"
 
 using namespace aceapex;
 
+enum KernelId { K_SCAN = 0, K_ENTROPY, K_MATCH, K_EXPORT, K_SEEK_INIT, K_SEEK_COLLECT, K_PARSE, K_SEEK_RESOLVE,
+                K_SEEK_CHECK, K_COUNT };
+static const char *const kKernelNames[K_COUNT] = { "k_scan_records", "k_entropy", "k_match", "k_export_streams",
+                                                   "k_seek_init", "k_seek_collect", "k_parse", "k_seek_resolve",
+                                                   "k_seek_check" };
+static_assert(K_COUNT <= ACEAPEX_N_KERNELS, "kernel id table");
+
+struct ProfRec { int id; cudaEvent_t e0, e1; };
+
 struct aceapex_ctx {
-    Container cv;
-    aceapex_info info;
-    SlotLayout sl;
-    Scratch sc;
-    bool have_scratch;
-    Control *open_ctl;          // tiny internal allocation used by the open-time scan
-    unsigned long long *h_pending;  // pinned, hop-loop read-back
-    uint32_t epoch, tag;
-    uint64_t launches;
-    int sm_count;
-    int device;
+    Container cv{};
+    aceapex_info info{};
+    SlotLayout sl{};
+    Scratch sc{};
+    bool have_scratch = false;
+    Control *open_ctl = nullptr;          // tiny internal allocation used by the open-time scan
+    unsigned long long *h_pending = nullptr;  // pinned, hop-loop read-back
+    uint32_t epoch = 0, tag = 0;
+    uint64_t launches = 0;
+    int sm_count = 0;
+    int device = 0;
+    bool prof = false;
+    std::vector<ProfRec> prof_recs;
+    std::vector<cudaEvent_t> prof_pool;
+};
+
+// Bracket one kernel launch: counts it and, while profiling, records an event pair around it.
+struct LaunchScope {
+    aceapex_ctx *c; cudaStream_t st; bool on;
+    LaunchScope(aceapex_ctx *c_, int id, cudaStream_t st_) : c(c_), st(st_), on(c_->prof)
+    {
+        c->launches++;
+        if (!on) return;
+        ProfRec r; r.id = id;
+        for (cudaEvent_t *e : { &r.e0, &r.e1 }) {
+            if (!c->prof_pool.empty()) { *e = c->prof_pool.back(); c->prof_pool.pop_back(); }
+            else if (cudaEventCreate(e) != cudaSuccess) { on = false; return; }
+        }
+        cudaEventRecord(r.e0, st);
+        c->prof_recs.push_back(r);
+    }
+    ~LaunchScope() { if (on) cudaEventRecord(c->prof_recs.back().e1, st); }
 };
 
 namespace {
@@ -70,9 +101,11 @@ int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list,
     uint32_t cap = (uint32_t)c->sm_count * 3;
     if (grid > cap) grid = cap;
     if (grid == 0) return ACEAPEX_OK;
-    k_entropy<<<grid, 128, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
-                                                 c->sc.ctl);
-    c->launches++;
+    {
+        LaunchScope ls(c, K_ENTROPY, st);
+        k_entropy<<<grid, 128, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
+                                                     c->sc.ctl);
+    }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
 }
 
@@ -123,7 +156,6 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
 
     aceapex_ctx *c = new (std::nothrow) aceapex_ctx();
     if (!c) return ACEAPEX_E_NOMEM;
-    memset(c, 0, sizeof *c);
     c->device = dev;
     const uint8_t *base = static_cast<const uint8_t *>(d_container);
     c->cv.base = base;
@@ -191,6 +223,8 @@ void aceapex_close(aceapex_ctx *c)
     if (!c) return;
     if (c->open_ctl) cudaFree(c->open_ctl);
     if (c->h_pending) cudaFreeHost(c->h_pending);
+    for (ProfRec &r : c->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     delete c;
 }
 
@@ -252,10 +286,12 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);
         int rc = launch_entropy(c, nullptr, nullptr, 0, first, count, st);
         if (rc != ACEAPEX_OK) return rc;
-        k_match<<<count, kMatchThreads, match_smem(c->sl), st>>>(c->cv, c->sl, c->sc.slots, first, count,
-                                                                static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
-                                                                c->sc.done, c->epoch);
-        c->launches++;
+        {
+            LaunchScope ls(c, K_MATCH, st);
+            k_match<<<count, kMatchThreads, match_smem(c->sl), st>>>(c->cv, c->sl, c->sc.slots, first, count,
+                                                                    static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
+                                                                    c->sc.done, c->epoch);
+        }
         if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
     }
     return ACEAPEX_OK;
@@ -272,10 +308,12 @@ int aceapex_decode_streams(aceapex_ctx *c, uint64_t first, size_t count, void *d
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int rc = launch_entropy(c, nullptr, nullptr, 0, first, (uint32_t)count, st);
     if (rc != ACEAPEX_OK) return rc;
-    k_export_streams<<<(uint32_t)count, 256, 0, st>>>(c->cv, c->sl, c->sc.slots, first, (uint32_t)count,
-                                                      static_cast<uint8_t *>(d_lit), static_cast<uint8_t *>(d_len),
-                                                      static_cast<uint8_t *>(d_off));
-    c->launches++;
+    {
+        LaunchScope ls(c, K_EXPORT, st);
+        k_export_streams<<<(uint32_t)count, 256, 0, st>>>(c->cv, c->sl, c->sc.slots, first, (uint32_t)count,
+                                                          static_cast<uint8_t *>(d_lit), static_cast<uint8_t *>(d_len),
+                                                          static_cast<uint8_t *>(d_off));
+    }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
 }
 
@@ -302,8 +340,10 @@ int aceapex_decode_blocks(aceapex_ctx *c, const uint64_t *h_ids, size_t n_ids, v
         const uint64_t n_bytes = (uint64_t)nt * kB;
         if (cudaMemcpyAsync(c->sc.ids, h_ids + base, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess)
             return ACEAPEX_E_CUDA;
-        k_seek_init<<<(uint32_t)((n_bytes + 255) / 256), 256, 0, st>>>(c->cv, c->sc.ids, nt, c->sc.pend);
-        c->launches++;
+        {
+            LaunchScope ls(c, K_SEEK_INIT, st);
+            k_seek_init<<<(uint32_t)((n_bytes + 255) / 256), 256, 0, st>>>(c->cv, c->sc.ids, nt, c->sc.pend);
+        }
         // With a depth promise D and a slot for every block a hop can touch, D+1 hops always
         // suffice (hop 0 resolves the target's own literals): enqueue them without reading back.
         const uint64_t touch = n_bytes < c->cv.n_blocks ? n_bytes : c->cv.n_blocks;
@@ -317,23 +357,29 @@ int aceapex_decode_blocks(aceapex_ctx *c, const uint64_t *h_ids, size_t n_ids, v
             }
             if (cudaMemsetAsync(&ctl->n_list, 0, 4, st) != cudaSuccess) return ACEAPEX_E_CUDA;
             if (cudaMemsetAsync(&ctl->pending, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-            k_seek_collect<<<cgrid, 128, 0, st>>>(c->sc.pend, n_bytes, c->sc.mark, c->sc.slot_of, c->sc.list, ctl,
-                                                  c->tag, S);
-            c->launches++;
+            {
+                LaunchScope ls(c, K_SEEK_COLLECT, st);
+                k_seek_collect<<<cgrid, 128, 0, st>>>(c->sc.pend, n_bytes, c->sc.mark, c->sc.slot_of, c->sc.list, ctl,
+                                                      c->tag, S);
+            }
             int rc = launch_entropy(c, c->sc.list, &ctl->n_list, S, 0, 0, st);
             if (rc != ACEAPEX_OK) return rc;
             uint32_t pgrid = S < (uint32_t)c->sm_count * 8 ? S : (uint32_t)c->sm_count * 8;
-            k_parse<<<pgrid, kMatchThreads, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.list, &ctl->n_list, S, ctl);
-            c->launches++;
-            k_seek_resolve<<<cgrid, 128, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.pend, nt, c->sc.ids, c->sc.mark,
-                                                  c->sc.slot_of, ctl, c->tag, S, static_cast<uint8_t *>(d_out),
-                                                  (uint64_t)base, absolute ? 1u : 0u);
-            c->launches++;
+            {
+                LaunchScope ls(c, K_PARSE, st);
+                k_parse<<<pgrid, kMatchThreads, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.list, &ctl->n_list, S, ctl);
+            }
+            {
+                LaunchScope ls(c, K_SEEK_RESOLVE, st);
+                k_seek_resolve<<<cgrid, 128, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.pend, nt, c->sc.ids, c->sc.mark,
+                                                      c->sc.slot_of, ctl, c->tag, S, static_cast<uint8_t *>(d_out),
+                                                      (uint64_t)base, absolute ? 1u : 0u);
+            }
             if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
             if (fixed) {
                 if (hop >= c->cv.D) {
+                    LaunchScope ls(c, K_SEEK_CHECK, st);
                     k_seek_check<<<1, 1, 0, st>>>(ctl);
-                    c->launches++;
                     break;
                 }
             } else {
@@ -377,5 +423,35 @@ int aceapex_device_status(aceapex_ctx *c, void *cuda_stream, uint64_t *first_bad
 }
 
 uint64_t aceapex_launch_count(const aceapex_ctx *c) { return c ? c->launches : 0; }
+
+int aceapex_profile_enable(aceapex_ctx *c, int on)
+{
+    if (!c) return ACEAPEX_E_ARG;
+    c->prof = on != 0;
+    return ACEAPEX_OK;
+}
+
+int aceapex_profile_read(aceapex_ctx *c, uint64_t *launches, double *ms)
+{
+    if (!c) return ACEAPEX_E_ARG;
+    if (cudaDeviceSynchronize() != cudaSuccess) return ACEAPEX_E_CUDA;
+    for (int i = 0; i < ACEAPEX_N_KERNELS; i++) {
+        if (launches) launches[i] = 0;
+        if (ms) ms[i] = 0.0;
+    }
+    int rc = ACEAPEX_OK;
+    for (ProfRec &r : c->prof_recs) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, r.e0, r.e1) != cudaSuccess) rc = ACEAPEX_E_CUDA;
+        if (launches) launches[r.id]++;
+        if (ms) ms[r.id] += (double)t;
+        c->prof_pool.push_back(r.e0);
+        c->prof_pool.push_back(r.e1);
+    }
+    c->prof_recs.clear();
+    return rc;
+}
+
+const char *aceapex_kernel_name(int id) { return id >= 0 && id < K_COUNT ? kKernelNames[id] : nullptr; }
 
 }  // extern "C"

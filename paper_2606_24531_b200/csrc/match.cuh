@@ -131,16 +131,30 @@ __device__ inline void st_release_u32(uint32_t *p, uint32_t v)
 }
 
 // Advance the watermark over every leading block whose done flag carries this call's epoch.
-__device__ inline void advance_watermark(Control *ctl, const uint32_t *done, uint64_t n_blocks, uint32_t epoch)
+// Called by all 32 lanes of one warp: 32 flags are examined per round trip. Returns the new
+// watermark (warp-uniform). The flags were read with acquire semantics and the fence orders them
+// before the atomicMax, so whoever later acquires the watermark also sees those blocks' bytes.
+__device__ inline unsigned long long advance_watermark(Control *ctl, const uint32_t *done, uint64_t n_blocks,
+                                                       uint32_t epoch)
 {
+    const uint32_t lane = lane_id();
+    unsigned long long w0 = 0;
+    if (lane == 0) w0 = ld_acquire_u64(&ctl->watermark);
+    w0 = __shfl_sync(0xFFFFFFFFu, w0, 0);
+    unsigned long long w = w0;
     for (;;) {
-        const unsigned long long w = ld_acquire_u64(&ctl->watermark);
-        if (w >= n_blocks) return;
-        if (ld_acquire_u32(done + w) != epoch) return;
-        unsigned long long old;
-        asm volatile("atom.acq_rel.gpu.global.cas.b64 %0, [%1], %2, %3;"
-                     : "=l"(old) : "l"(&ctl->watermark), "l"(w), "l"(w + 1) : "memory");
+        const unsigned long long idx = w + lane;
+        const bool f = idx < n_blocks && ld_acquire_u32(done + idx) == epoch;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
+        const uint32_t c = m == 0xFFFFFFFFu ? 32u : (uint32_t)__ffs(~m) - 1u;
+        w += c;
+        if (c < 32) break;
     }
+    if (w > w0 && lane == 0) {
+        __threadfence();
+        atomicMax(&ctl->watermark, w);
+    }
+    return w;
 }
 
 // decode_all, match layer. One CTA per block; block ids are handed out in increasing order by a
@@ -204,11 +218,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             // wait until every earlier block this block copies from is complete
             const uint64_t below = s_below;                  // 1 + highest earlier block read
             if (below) {
-                if (threadIdx.x == 0) {
-                    while (ld_acquire_u64(&ctl->watermark) < below) {
-                        advance_watermark(ctl, done, cv.n_blocks, epoch);
-                        __nanosleep(100);
-                    }
+                if (warp == 0) {
+                    while (advance_watermark(ctl, done, cv.n_blocks, epoch) < below) __nanosleep(64);
                     __threadfence();
                 }
                 __syncthreads();
@@ -244,8 +255,9 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         // publish (also for a bad block: later blocks must not wait forever)
         __threadfence();
         __syncthreads();
-        if (threadIdx.x == 0) {
-            st_release_u32(done + blk, epoch);
+        if (threadIdx.x < 32) {
+            if (threadIdx.x == 0) st_release_u32(done + blk, epoch);
+            __syncwarp();
             advance_watermark(ctl, done, cv.n_blocks, epoch);
         }
     }
