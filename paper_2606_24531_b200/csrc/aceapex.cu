@@ -90,20 +90,20 @@ inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
     return rest < kB ? (uint32_t)rest : kB;
 }
 
-inline size_t entropy_smem() { return 4 * kEntropyWarpSmemWords * sizeof(uint32_t); }
-inline size_t match_smem(const SlotLayout &sl) { return kB + 15 * (size_t)sl.ms + 64; }
+inline size_t entropy_smem() { return (size_t)kEntropyWarps * kEntropyWarpSmem; }
+inline size_t match_smem(const SlotLayout &sl) { return kB + 3072 + 15 * (size_t)sl.ms + 64; }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                    uint32_t count, cudaStream_t st)
 {
     uint32_t units = 3 * (list ? max_slots : count);
-    uint32_t grid = (units + 3) / 4;
-    uint32_t cap = (uint32_t)c->sm_count * 3;
+    uint32_t grid = (units + kEntropyWarps - 1) / kEntropyWarps;
+    uint32_t cap = (uint32_t)c->sm_count * 4;
     if (grid > cap) grid = cap;
     if (grid == 0) return ACEAPEX_OK;
     {
         LaunchScope ls(c, K_ENTROPY, st);
-        k_entropy<<<grid, 128, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
+        k_entropy<<<grid, 32 * kEntropyWarps, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
                                                      c->sc.ctl);
     }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;

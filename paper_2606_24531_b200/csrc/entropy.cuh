@@ -10,9 +10,17 @@
 
 namespace aceapex {
 
-constexpr uint32_t kTblWords = kM;          // packed decode table: one u32 per slot
-constexpr uint32_t kSymListWords = 256;     // present symbols, packed
-constexpr uint32_t kEntropyWarpSmemWords = kTblWords + kSymListWords;
+// Per-warp shared memory of the entropy decoder (bytes):
+//   t8   [4096]  slot -> index of the present symbol that owns the slot
+//   syml [256]   u64 per present symbol: lo = sym | (-c) << 8 (two's complement, 24 bit), hi = f
+//   aux  [768]   table build: 4096-bit boundary bitmap (512 B) + u16 rank per bitmap word (256 B);
+//                decode: ring of 256 16-bit rANS words (512 B), refilled with cp.async
+constexpr uint32_t kT8Bytes = kM;
+constexpr uint32_t kSymlBytes = 256 * 8;
+constexpr uint32_t kAuxBytes = 768;
+constexpr uint32_t kEntropyWarpSmem = kT8Bytes + kSymlBytes + kAuxBytes;   // 6912
+constexpr uint32_t kEntropyWarps = 8;
+constexpr uint32_t kRingWords = 256, kRingChunk = 64;
 
 __device__ inline uint32_t lane_id() { return threadIdx.x & 31u; }
 
@@ -28,11 +36,23 @@ __device__ inline uint32_t warp_excl_scan(uint32_t v, uint32_t lane, uint32_t &t
     return inc - v;
 }
 
-// Build the 4096-entry packed decode table of one stream in shared memory.
-// entry = sym | (f-1) << 8 | (slot - c[sym]) << 20, so that x' = f*(x>>12) + (slot - c).
-// Returns false (warp-uniform) if the table section is invalid (FORMAT.md section 3 "Table").
-__device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, uint32_t *tbl, uint32_t *syml,
-                                   uint32_t lane)
+__device__ inline void cp_async4(void *smem_dst, const void *gsrc)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ inline void cp_async16(void *smem_dst, const void *gsrc)
+{
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ inline void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ inline void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Build the two-level decode table of one stream in shared memory (FORMAT.md section 3 "Table").
+// Returns false (warp-uniform) if the table section is invalid.
+__device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, uint8_t *t8, uint2 *syml,
+                                   uint32_t *bmw /* [128] */, uint16_t *rk /* [128] */, uint32_t lane)
 {
     if (tbl_bytes < 32) return false;
     const uint32_t bm = tbl_sec[lane];                   // presence of symbols 8*lane .. 8*lane+7
@@ -54,65 +74,125 @@ __device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, u
             }
         }
     }
-    if (__any_sync(0xFFFFFFFFu, bad)) return false;      // also bounds every f before the scan
+    if (__any_sync(0xFFFFFFFFu, bad)) return false;      // bounds every f before the scan
     uint32_t total;
     uint32_t c = warp_excl_scan(sum, lane, total);
     if (total != kM) return false;
+    reinterpret_cast<uint4 *>(bmw)[lane] = make_uint4(0, 0, 0, 0);
+    __syncwarp();
     {
         uint32_t j = first;
 #pragma unroll
         for (int k = 0; k < 8; k++)
             if (bm >> k & 1u) {
-                syml[j++] = (8 * lane + k) | (f[k] - 1) << 8 | c << 20;   // c <= 4095
+                syml[j++] = make_uint2((8 * lane + k) | (0u - c) << 8, f[k]);   // c <= 4095
+                atomicOr(&bmw[c >> 5], 1u << (c & 31));                          // symbol starts at slot c
                 c += f[k];
             }
     }
     __syncwarp();
-    for (uint32_t j = 0; j < n_present; j++) {
-        const uint32_t e = syml[j];
-        const uint32_t fm1 = (e >> 8) & 0xFFFu, c0 = e >> 20, lo = e & 0xFFFFFu;
-        for (uint32_t k = lane; k <= fm1; k += 32) tbl[c0 + k] = lo | k << 20;
+    {   // rank of each bitmap word = number of symbol starts in the words before it
+        const uint4 w = reinterpret_cast<const uint4 *>(bmw)[lane];
+        const uint32_t p0 = __popc(w.x), p1 = __popc(w.y), p2 = __popc(w.z), p3 = __popc(w.w);
+        uint32_t tot;
+        const uint32_t r0 = warp_excl_scan(p0 + p1 + p2 + p3, lane, tot);
+        reinterpret_cast<uint2 *>(rk)[lane] = make_uint2(r0 | (r0 + p0) << 16, (r0 + p0 + p1) | (r0 + p0 + p1 + p2) << 16);
+    }
+    __syncwarp();
+    // fill: per iteration the warp writes 512 slots, 16 consecutive bytes per lane
+#pragma unroll 2
+    for (uint32_t it = 0; it < 8; it++) {
+        const uint32_t wi = 16 * it + (lane >> 1), h = (lane & 1u) * 16;
+        const uint32_t w = bmw[wi];
+        const uint32_t bits = (w >> h) & 0xFFFFu;
+        // index of the symbol that owns the slot just before this lane's first slot
+        uint32_t base = (uint32_t)rk[wi] + __popc(w & ((1u << h) - 1u)) - 1u;
+        uint32_t o[4];
+#pragma unroll
+        for (int g = 0; g < 4; g++) {
+            const uint32_t nib = (bits >> (4 * g)) & 0xFu;
+            const uint32_t spread = (nib * 0x00204081u) & 0x01010101u;   // bit k -> byte k
+            o[g] = spread * 0x01010101u + base * 0x01010101u;            // running symbol index per slot
+            base = o[g] >> 24;
+        }
+        reinterpret_cast<uint4 *>(t8)[32 * it + lane] = make_uint4(o[0], o[1], o[2], o[3]);
     }
     __syncwarp();
     return true;
 }
 
-// Decode stream s of block `blk` into out[0, n_sym). One warp. Returns true (warp-uniform) on
-// success; false if the table or the rANS end conditions are violated (then out is unspecified
-// but never written beyond n_sym).
-__device__ inline bool decode_stream(const Container &cv, const Record &r, int s, uint64_t blk, uint8_t *out,
-                                     uint32_t *tbl, uint32_t *syml, uint32_t lane)
+// Decode one stream (n symbols, n_words 16-bit words) into out[0, n). One warp. Returns true
+// (warp-uniform) on success; false if the table or the rANS end conditions are violated (then
+// out is unspecified but never written beyond n).
+__device__ inline bool decode_stream(uint32_t x /* this lane's initial state */, uint32_t n, uint32_t n_words,
+                                     const uint8_t *tbl_sec, uint32_t tbl_bytes, const uint8_t *words_sec,
+                                     uint8_t *out, uint8_t *wsm, uint32_t lane)
 {
-    const uint32_t n = r.n_sym[s], n_words = r.n_words[s];
-    uint32_t x = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
     if (n == 0) return __all_sync(0xFFFFFFFFu, x == kRansL) && n_words == 0;
-    if (!build_table(r.rec + r.tbl_off[s], r.tbl_bytes[s], tbl, syml, lane)) return false;
-    const uint16_t *words = reinterpret_cast<const uint16_t *>(r.rec + r.words_off[s]);
+    uint8_t *t8 = wsm;
+    uint2 *syml = reinterpret_cast<uint2 *>(wsm + kT8Bytes);
+    uint8_t *aux = wsm + kT8Bytes + kSymlBytes;
+    __syncwarp();
+    if (!build_table(tbl_sec, tbl_bytes, t8, syml, reinterpret_cast<uint32_t *>(aux),
+                     reinterpret_cast<uint16_t *>(aux + 512), lane))
+        return false;
+    // word ring: 4 chunks of 64 words; chunk k lives at ring[(k & 3) * 64 ...]
+    uint16_t *ring = reinterpret_cast<uint16_t *>(aux);
+    const uint32_t wbytes = 2 * n_words;
+    if (16 * lane < wbytes) cp_async16(aux + 16 * lane, words_sec + 16 * lane);   // words 0 .. 255
+    cp_async_commit();
+    cp_async_wait_all();
+    __syncwarp();
     const uint32_t lt = (1u << lane) - 1u;
-    uint32_t wpos = 0;
+    uint32_t wpos = 0, trigger = kRingChunk;
     bool overrun = false;
-    const uint32_t rounds = (n + 31u) >> 5;
-    for (uint32_t rd = 0; rd < rounds; rd++) {
-        const uint32_t i = (rd << 5) + lane;
-        const bool active = i < n;
+    const uint32_t full = n >> 5;
+    for (uint32_t rd = 0; rd < full; rd++) {
+        if (wpos >= trigger) {
+            // the chunk requested at the previous trigger has had >= 64 words of decoding to land
+            cp_async_wait_all();
+            __syncwarp();
+            const uint32_t chunk = trigger / kRingChunk + 3;         // next chunk that is not resident
+            const uint32_t boff = chunk * (2 * kRingChunk) + 4 * lane;
+            if (boff < wbytes) cp_async4(aux + ((chunk & 3u) * (2 * kRingChunk) + 4 * lane), words_sec + boff);
+            cp_async_commit();
+            trigger += kRingChunk;
+        }
+        const uint32_t slot = x & (kM - 1);
+        const uint2 e = syml[t8[slot]];
+        x = e.y * (x >> kProbBits) + (slot + (uint32_t)((int32_t)e.x >> 8));
+        const bool need = x < kRansL;
+        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, need);
+        if (need) {
+            const uint32_t idx = wpos + __popc(mask & lt);
+            if (idx >= n_words) overrun = true;
+            x = (x << 16) | ring[idx & (kRingWords - 1)];
+        }
+        wpos += __popc(mask);
+        out[(rd << 5) + lane] = (uint8_t)e.x;
+    }
+    if (n & 31u) {                                                   // ragged last round
+        if (wpos >= trigger) { cp_async_wait_all(); __syncwarp(); }
+        const bool active = lane < (n & 31u);
         bool need = false;
         uint32_t sym = 0;
         if (active) {
-            const uint32_t e = tbl[x & (kM - 1)];
-            sym = e & 0xFFu;
-            x = (((e >> 8) & 0xFFFu) + 1u) * (x >> kProbBits) + (e >> 20);
+            const uint32_t slot = x & (kM - 1);
+            const uint2 e = syml[t8[slot]];
+            sym = e.x;
+            x = e.y * (x >> kProbBits) + (slot + (uint32_t)((int32_t)e.x >> 8));
             need = x < kRansL;
         }
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, need);
         if (need) {
             const uint32_t idx = wpos + __popc(mask & lt);
-            uint32_t w = 0;
-            if (idx < n_words) w = __ldg(words + idx); else overrun = true;
-            x = (x << 16) | w;
+            if (idx >= n_words) overrun = true;
+            x = (x << 16) | ring[idx & (kRingWords - 1)];
         }
         wpos += __popc(mask);
-        if (active) out[i] = (uint8_t)sym;
+        if (active) out[(full << 5) + lane] = (uint8_t)sym;
     }
+    cp_async_wait_all();
     const bool good = !overrun && x == kRansL;
     return __all_sync(0xFFFFFFFFu, good) && wpos == n_words;
 }
@@ -121,14 +201,13 @@ __device__ inline bool decode_stream(const Container &cv, const Record &r, int s
 //   list != nullptr: the blocks are list[0 .. min(*n_list, max_slots)) (isolated path);
 //   else:            the blocks are first .. first+count-1.
 // Unit u -> block index u/3 (= slot), stream u%3. Output: the slot's LIT/LEN/OFF areas.
-__global__ void __launch_bounds__(128) k_entropy(Container cv, SlotLayout sl, uint8_t *slots, const uint64_t *list,
+__global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, SlotLayout sl, uint8_t *slots, const uint64_t *list,
                                                  const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                                                  uint32_t count, Control *ctl)
 {
-    extern __shared__ uint32_t smem_u32[];
+    extern __shared__ __align__(16) uint8_t smem_entropy[];
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-    uint32_t *tbl = smem_u32 + warp * kEntropyWarpSmemWords;
-    uint32_t *syml = tbl + kTblWords;
+    uint8_t *wsm = smem_entropy + warp * kEntropyWarpSmem;
     uint32_t nb = count;
     if (list) { nb = *n_list; if (nb > max_slots) nb = max_slots; }
     const uint32_t n_units = 3 * nb;
@@ -148,11 +227,18 @@ __global__ void __launch_bounds__(128) k_entropy(Container cv, SlotLayout sl, ui
             // a stream longer than its slot area cannot occur once open() has found max_n_seq,
             // but the check keeps the store loop in bounds for any input
             const uint32_t cap = s == LIT ? kB : (s == LEN ? 2 * sl.ms : cv.W * sl.ms);
-            if (r.n_sym[s] > cap) ok = false;
+            const uint32_t ns = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
+            if (ns > cap) ok = false;
         }
         if (ok) {
             uint8_t *out = slot + (s == LIT ? sl.o_lit : (s == LEN ? sl.o_len : sl.o_off));
-            ok = decode_stream(cv, r, s, blk, out, tbl, syml, lane);
+            const uint32_t n = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
+            const uint32_t nw = s == LIT ? r.n_words[LIT] : (s == LEN ? r.n_words[LEN] : r.n_words[OFF]);
+            const uint32_t to = s == LIT ? r.tbl_off[LIT] : (s == LEN ? r.tbl_off[LEN] : r.tbl_off[OFF]);
+            const uint32_t tb = s == LIT ? r.tbl_bytes[LIT] : (s == LEN ? r.tbl_bytes[LEN] : r.tbl_bytes[OFF]);
+            const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
+            const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
+            ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, wsm, lane);
             if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
         } else if (lane == 0) {
             raise(ctl, kStRecord, blk);

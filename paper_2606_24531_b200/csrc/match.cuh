@@ -16,6 +16,7 @@ struct Tokens {
     uint16_t *dst;     // [n_seq]   in-block output offset of match k
     uint16_t *litpos;  // [n_seq+1] index into LIT of sequence k's first literal
     uint64_t *src;     // [n_seq]   absolute source position of match k
+    uint32_t *bm;      // optional [512]: bit o set iff some sequence (or the trailing run) starts at offset o
 };
 
 // Exclusive prefix sum of one value per thread over the CTA (kMatchThreads threads).
@@ -88,6 +89,7 @@ __device__ inline bool parse_tokens(const Record &r, uint64_t blk, const uint8_t
             for (uint32_t j = 0; j < r.off_nbytes; j++) src |= (uint64_t)off_s[k * r.off_nbytes + j] << (8 * j);
             t.start[k] = (uint16_t)pos;
             t.litpos[k] = (uint16_t)lp;
+            if (t.bm && pos < kB) atomicOr(&t.bm[pos >> 5], 1u << (pos & 31));
             pos += ll; lp += ll;
             t.dst[k] = (uint16_t)pos;
             t.src[k] = src;
@@ -103,6 +105,7 @@ __device__ inline bool parse_tokens(const Record &r, uint64_t blk, const uint8_t
     if (threadIdx.x == kMatchThreads - 1) {
         t.start[n] = (uint16_t)all_total;
         t.litpos[n] = (uint16_t)ll_total;
+        if (t.bm && all_total < kB) atomicOr(&t.bm[all_total >> 5], 1u << (all_total & 31));
     }
     if (max_src_blk_below) {
         // CTA-wide max via shared atomics; caller zeroed *max_src_blk_below before the call
@@ -157,9 +160,22 @@ __device__ inline unsigned long long advance_watermark(Control *ctl, const uint3
     return w;
 }
 
+// Source byte of a match at absolute position p: inside the block from the tile, else from the
+// output buffer (an earlier, completed block).
+__device__ inline uint32_t src_byte(const uint8_t *tile, const uint8_t *out, uint64_t B0, uint64_t p)
+{
+    return p >= B0 ? tile[p - B0] : out[p];
+}
+
 // decode_all, match layer. One CTA per block; block ids are handed out in increasing order by a
 // ticket, so a CTA only ever waits for blocks whose CTAs are already running or finished.
 //   slots: decoded streams of blocks first .. first+count-1 (slot i = block first+i).
+//
+// Pass 0 is output-centric: every thread produces groups of 4 consecutive output bytes. The
+// sequence that owns output offset o is rank[o>>5] + popc(bitmap word below o) - 1, where the
+// bitmap marks the start offset of every sequence: no search. Literal bytes come from the LIT
+// stream, bytes of tag-0 matches (source entirely in earlier blocks) from the output buffer.
+// Matches with tag >= 1 (source inside this block) follow level by level (FORMAT.md section 4).
 __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayout sl, const uint8_t *slots,
                                                           uint64_t first, uint32_t count, uint8_t *out,
                                                           uint32_t out_aligned16, Control *ctl, uint32_t *done,
@@ -172,11 +188,14 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     __shared__ uint32_t s_maxtag;
 
     uint8_t *tile = smem;                                    // 16384
+    uint32_t *bm = reinterpret_cast<uint32_t *>(smem + kB);  // 512 words
+    uint16_t *rank = reinterpret_cast<uint16_t *>(smem + kB + 2048);   // 512
     Tokens t;
-    t.src = reinterpret_cast<uint64_t *>(smem + kB);
-    t.start = reinterpret_cast<uint16_t *>(smem + kB + 8 * sl.ms);
+    t.src = reinterpret_cast<uint64_t *>(smem + kB + 3072);
+    t.start = reinterpret_cast<uint16_t *>(smem + kB + 3072 + 8 * sl.ms);
     t.dst = t.start + (sl.ms + 16);
     t.litpos = t.dst + sl.ms;
+    t.bm = bm;
     uint8_t *tags = reinterpret_cast<uint8_t *>(t.litpos + (sl.ms + 16));   // [ms]
 
     if (threadIdx.x == 0) {
@@ -184,6 +203,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         s_below = 0;
         s_maxtag = 0;
     }
+    for (uint32_t i = threadIdx.x; i < 512; i += kMatchThreads) bm[i] = 0;
     __syncthreads();
     const uint32_t bi = s_ticket;
     if (bi < count) {
@@ -198,7 +218,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             if (!ok && threadIdx.x == 0) raise(ctl, kStTokens, blk);
         }
         if (ok) {
-            const uint32_t n = r.n_seq;
+            const uint32_t n = r.n_seq, blen = r.block_len;
             const uint8_t *lit = slot + sl.o_lit;
             const uint8_t *tagsec = r.rec + r.tags_off;
             uint32_t mt = 0;
@@ -208,46 +228,77 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 mt = max(mt, tg);
             }
             if (mt) atomicMax(&s_maxtag, mt);
-            const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
-            // literal runs (sequence n = the trailing literals)
-            for (uint32_t k = warp; k <= n; k += kMatchWarps) {
-                const uint32_t a = t.start[k], b = k < n ? t.dst[k] : r.block_len, lp = t.litpos[k];
-                for (uint32_t j = a + lane; j < b; j += 32) tile[j] = lit[lp + (j - a)];
+            // rank[w] = number of sequence starts in bitmap words before w
+            {
+                uint32_t p0 = 0, p1 = 0, p2 = 0, p3 = 0;
+                if (threadIdx.x < 128) {
+                    const uint4 w = reinterpret_cast<const uint4 *>(bm)[threadIdx.x];
+                    p0 = __popc(w.x); p1 = __popc(w.y); p2 = __popc(w.z); p3 = __popc(w.w);
+                }
+                uint32_t tot;
+                const uint32_t r0 = block_excl_scan(p0 + p1 + p2 + p3, warp_sums, tot);
+                if (threadIdx.x < 128)
+                    reinterpret_cast<uint2 *>(rank)[threadIdx.x] =
+                        make_uint2(r0 | (r0 + p0) << 16, (r0 + p0 + p1) | (r0 + p0 + p1 + p2) << 16);
+            }
+            // wait until every earlier block this block copies from is complete
+            const uint32_t warp = threadIdx.x >> 5;
+            const uint64_t below = s_below;                  // 1 + highest earlier block read
+            if (below && warp == 0) {
+                while (advance_watermark(ctl, done, cv.n_blocks, epoch) < below) __nanosleep(64);
+                __threadfence();
             }
             __syncthreads();
-            // wait until every earlier block this block copies from is complete
-            const uint64_t below = s_below;                  // 1 + highest earlier block read
-            if (below) {
-                if (warp == 0) {
-                    while (advance_watermark(ctl, done, cv.n_blocks, epoch) < below) __nanosleep(64);
-                    __threadfence();
+            // pass 0: literals and tag-0 matches, 4 output bytes per thread per step
+            for (uint32_t o = 4 * threadIdx.x; o < blen; o += 4 * kMatchThreads) {
+                const uint32_t w = bm[o >> 5], sh = o & 31u;
+                const uint32_t q = (uint32_t)rank[o >> 5] + __popc(w & ((2u << sh) - 1u)) - 1u;
+                const uint32_t st = t.start[q], d = q < n ? t.dst[q] : blen;
+                uint32_t v = 0;
+                const bool one_seq = ((w >> sh) & 0xEu) == 0 && o + 4 <= blen;
+                if (one_seq && o + 4 <= d) {                 // four literal bytes of sequence q
+                    const uint8_t *p = lit + t.litpos[q] + (o - st);
+                    v = p[0] | p[1] << 8 | p[2] << 16 | p[3] << 24;
+                } else if (one_seq && o >= d) {              // four bytes of match q
+                    if (tags[q] == 0) {
+                        const uint8_t *p = out + t.src[q] + (o - d);
+                        v = p[0] | p[1] << 8 | p[2] << 16 | p[3] << 24;
+                    }
+                } else {                                     // a boundary inside the group
+                    uint32_t qq = q, s0 = st, dd = d;
+                    for (uint32_t j = 0; j < 4 && o + j < blen; j++) {
+                        const uint32_t oj = o + j;
+                        if (j && ((w >> (sh + j)) & 1u)) { qq++; s0 = oj; dd = qq < n ? t.dst[qq] : blen; }
+                        uint32_t b = 0;
+                        if (oj < dd) b = lit[t.litpos[qq] + (oj - s0)];
+                        else if (tags[qq] == 0) b = out[t.src[qq] + (oj - dd)];
+                        v |= b << (8 * j);
+                    }
                 }
-                __syncthreads();
+                *reinterpret_cast<uint32_t *>(tile + o) = v;
             }
-            // copies, level by level (FORMAT.md section 4 "tags")
+            __syncthreads();
+            // matches whose source lies (partly) inside this block, level by level
             const uint32_t maxtag = s_maxtag;
-            for (uint32_t level = 0; level <= maxtag; level++) {
-                for (uint32_t k = warp; k < n; k += kMatchWarps) {
+            for (uint32_t level = 1; level <= maxtag; level++) {
+                for (uint32_t k = threadIdx.x; k < n; k += kMatchThreads) {
                     if (tags[k] != level) continue;
                     const uint32_t d = t.dst[k], ml = t.start[k + 1] - d;
                     const uint64_t src = t.src[k];
-                    for (uint32_t j = lane; j < ml; j += 32) {
-                        const uint64_t p = src + j;
-                        tile[d + j] = p >= B0 ? tile[p - B0] : out[p];
-                    }
+                    for (uint32_t j = 0; j < ml; j++) tile[d + j] = (uint8_t)src_byte(tile, out, B0, src + j);
                 }
                 __syncthreads();
             }
             // tile -> output
             uint8_t *dstp = out + B0;
             if (out_aligned16) {
-                const uint32_t nvec = r.block_len >> 4;
+                const uint32_t nvec = blen >> 4;
                 const uint4 *tv = reinterpret_cast<const uint4 *>(tile);
                 uint4 *ov = reinterpret_cast<uint4 *>(dstp);
                 for (uint32_t i = threadIdx.x; i < nvec; i += kMatchThreads) ov[i] = tv[i];
-                for (uint32_t i = (nvec << 4) + threadIdx.x; i < r.block_len; i += kMatchThreads) dstp[i] = tile[i];
+                for (uint32_t i = (nvec << 4) + threadIdx.x; i < blen; i += kMatchThreads) dstp[i] = tile[i];
             } else {
-                for (uint32_t i = threadIdx.x; i < r.block_len; i += kMatchThreads) dstp[i] = tile[i];
+                for (uint32_t i = threadIdx.x; i < blen; i += kMatchThreads) dstp[i] = tile[i];
             }
         } else if (threadIdx.x == 0 && !r.ok) {
             raise(ctl, kStRecord, blk);
@@ -291,6 +342,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_parse(Container cv, SlotLayou
         t.dst = reinterpret_cast<uint16_t *>(slot + sl.o_dst);
         t.litpos = reinterpret_cast<uint16_t *>(slot + sl.o_litpos);
         t.src = reinterpret_cast<uint64_t *>(slot + sl.o_src);
+        t.bm = nullptr;
         if (ok) {
             ok = parse_tokens(r, blk, slot + sl.o_len, slot + sl.o_off, t, warp_sums, nullptr);
             if (!ok && threadIdx.x == 0) raise(ctl, kStTokens, blk);
