@@ -90,7 +90,7 @@ inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
     return rest < kB ? (uint32_t)rest : kB;
 }
 
-inline size_t entropy_smem() { return (size_t)kEntropyWarps * kEntropyWarpSmem; }
+inline size_t entropy_smem() { return kEntropySmem; }
 inline size_t match_smem(const SlotLayout &sl) { return kB + 3072 + 15 * (size_t)sl.ms + 64; }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
@@ -98,7 +98,7 @@ int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list,
 {
     uint32_t units = 3 * (list ? max_slots : count);
     uint32_t grid = (units + kEntropyWarps - 1) / kEntropyWarps;
-    uint32_t cap = (uint32_t)c->sm_count * 4;
+    uint32_t cap = (uint32_t)c->sm_count * 2;   // 2 CTAs of 16 warps per SM (shared memory)
     if (grid > cap) grid = cap;
     if (grid == 0) return ACEAPEX_OK;
     {

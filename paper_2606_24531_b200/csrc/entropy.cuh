@@ -10,17 +10,44 @@
 
 namespace aceapex {
 
-// Per-warp shared memory of the entropy decoder (bytes):
-//   t8   [4096]  slot -> index of the present symbol that owns the slot
+// Shared memory of the entropy decoder, per warp (bytes):
+//   t8   [4096]  slot -> index of the present symbol that owns the slot. All t8 tables of a CTA sit in
+//                one 4096-aligned region of the shared window, so a lookup address is
+//                (x & 4095) | t8_base: one LOP3.
 //   syml [256]   u64 per present symbol: lo = sym | (-c) << 8 (two's complement, 24 bit), hi = f
-//   aux  [768]   table build: 4096-bit boundary bitmap (512 B) + u16 rank per bitmap word (256 B);
-//                decode: ring of 256 16-bit rANS words (512 B), refilled with cp.async
+//   ring [512]   table build: 4096-bit symbol-start bitmap; decode: ring of 256 16-bit rANS words,
+//                refilled with cp.async. (The build's 256-byte rank array borrows the tail of t8.)
 constexpr uint32_t kT8Bytes = kM;
 constexpr uint32_t kSymlBytes = 256 * 8;
-constexpr uint32_t kAuxBytes = 768;
-constexpr uint32_t kEntropyWarpSmem = kT8Bytes + kSymlBytes + kAuxBytes;   // 6912
-constexpr uint32_t kEntropyWarps = 8;
+constexpr uint32_t kRingBytes = 512;
+constexpr uint32_t kEntropyWarps = 16;
+constexpr uint32_t kEntropySmem = kEntropyWarps * (kT8Bytes + kSymlBytes + kRingBytes) + kT8Bytes;   // + alignment slack
 constexpr uint32_t kRingWords = 256, kRingChunk = 64;
+
+// Where one warp's tables live: generic pointers for the build, shared-window addresses for the loop.
+struct WarpSmem {
+    uint8_t *t8; uint2 *syml; uint8_t *ring;
+    uint32_t a_t8, a_syml, a_ring;
+};
+
+__device__ inline uint32_t lds_u8(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ inline uint32_t lds_u16(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ inline uint2 lds_v2(uint32_t a)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
 
 __device__ inline uint32_t lane_id() { return threadIdx.x & 31u; }
 
@@ -52,7 +79,8 @@ __device__ inline void cp_async_wait_all() { asm volatile("cp.async.wait_group 0
 // Build the two-level decode table of one stream in shared memory (FORMAT.md section 3 "Table").
 // Returns false (warp-uniform) if the table section is invalid.
 __device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, uint8_t *t8, uint2 *syml,
-                                   uint32_t *bmw /* [128] */, uint16_t *rk /* [128] */, uint32_t lane)
+                                   uint32_t *bmw /* [128] */, uint16_t *rk /* [128], may alias t8[3840..] */,
+                                   uint32_t lane)
 {
     if (tbl_bytes < 32) return false;
     const uint32_t bm = tbl_sec[lane];                   // presence of symbols 8*lane .. 8*lane+7
@@ -107,6 +135,7 @@ __device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, u
         const uint32_t bits = (w >> h) & 0xFFFFu;
         // index of the symbol that owns the slot just before this lane's first slot
         uint32_t base = (uint32_t)rk[wi] + __popc(w & ((1u << h) - 1u)) - 1u;
+        __syncwarp();                                    // rk borrows the tail of t8: read before the last write
         uint32_t o[4];
 #pragma unroll
         for (int g = 0; g < 4; g++) {
@@ -121,93 +150,124 @@ __device__ inline bool build_table(const uint8_t *tbl_sec, uint32_t tbl_bytes, u
     return true;
 }
 
+// One rANS round of the warp (FORMAT.md section 3), branch-free: decode this lane's symbol, then the
+// lanes whose state fell below 2^16 take consecutive words in lane order. wpos2 = 2 * words consumed.
+#define ACEAPEX_RANS_ROUND(SYM)                                                                        \
+    {                                                                                                  \
+        const uint32_t slot_ = x & (kM - 1);                                                           \
+        const uint32_t i_ = lds_u8(slot_ | ws.a_t8);                                                   \
+        const uint2 e_ = lds_v2(i_ * 8u + ws.a_syml);                                                  \
+        x = e_.y * (x >> kProbBits) + (slot_ + (uint32_t)((int32_t)e_.x >> 8));                        \
+        const bool need_ = x < kRansL;                                                                 \
+        const uint32_t mask_ = __ballot_sync(0xFFFFFFFFu, need_);                                      \
+        const uint32_t w_ = lds_u16(((wpos2 + 2u * __popc(mask_ & lt)) & (2 * kRingWords - 1)) | ws.a_ring); \
+        if (need_) x = (x << 16) | w_;                                                                 \
+        wpos2 += 2u * __popc(mask_);                                                                   \
+        SYM = e_.x;                                                                                    \
+    }
+
 // Decode one stream (n symbols, n_words 16-bit words) into out[0, n). One warp. Returns true
 // (warp-uniform) on success; false if the table or the rANS end conditions are violated (then
-// out is unspecified but never written beyond n).
+// out is unspecified but never written beyond n). A stream that consumes more words than it has
+// reads stale ring entries (shared memory, in bounds) and fails the final word-count check.
 __device__ inline bool decode_stream(uint32_t x /* this lane's initial state */, uint32_t n, uint32_t n_words,
                                      const uint8_t *tbl_sec, uint32_t tbl_bytes, const uint8_t *words_sec,
-                                     uint8_t *out, uint8_t *wsm, uint32_t lane)
+                                     uint8_t *out, const WarpSmem &ws, uint32_t lane)
 {
     if (n == 0) return __all_sync(0xFFFFFFFFu, x == kRansL) && n_words == 0;
-    uint8_t *t8 = wsm;
-    uint2 *syml = reinterpret_cast<uint2 *>(wsm + kT8Bytes);
-    uint8_t *aux = wsm + kT8Bytes + kSymlBytes;
     __syncwarp();
-    if (!build_table(tbl_sec, tbl_bytes, t8, syml, reinterpret_cast<uint32_t *>(aux),
-                     reinterpret_cast<uint16_t *>(aux + 512), lane))
+    if (!build_table(tbl_sec, tbl_bytes, ws.t8, ws.syml, reinterpret_cast<uint32_t *>(ws.ring),
+                     reinterpret_cast<uint16_t *>(ws.t8 + kT8Bytes - 256), lane))
         return false;
     // word ring: 4 chunks of 64 words; chunk k lives at ring[(k & 3) * 64 ...]
-    uint16_t *ring = reinterpret_cast<uint16_t *>(aux);
     const uint32_t wbytes = 2 * n_words;
-    if (16 * lane < wbytes) cp_async16(aux + 16 * lane, words_sec + 16 * lane);   // words 0 .. 255
+    if (16 * lane < wbytes) cp_async16(ws.ring + 16 * lane, words_sec + 16 * lane);   // words 0 .. 255
     cp_async_commit();
     cp_async_wait_all();
     __syncwarp();
     const uint32_t lt = (1u << lane) - 1u;
-    uint32_t wpos = 0, trigger = kRingChunk;
-    bool overrun = false;
-    const uint32_t full = n >> 5;
-    for (uint32_t rd = 0; rd < full; rd++) {
-        if (wpos >= trigger) {
-            // the chunk requested at the previous trigger has had >= 64 words of decoding to land
-            cp_async_wait_all();
-            __syncwarp();
-            const uint32_t chunk = trigger / kRingChunk + 3;         // next chunk that is not resident
-            const uint32_t boff = chunk * (2 * kRingChunk) + 4 * lane;
-            if (boff < wbytes) cp_async4(aux + ((chunk & 3u) * (2 * kRingChunk) + 4 * lane), words_sec + boff);
-            cp_async_commit();
-            trigger += kRingChunk;
-        }
-        const uint32_t slot = x & (kM - 1);
-        const uint2 e = syml[t8[slot]];
-        x = e.y * (x >> kProbBits) + (slot + (uint32_t)((int32_t)e.x >> 8));
-        const bool need = x < kRansL;
-        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, need);
-        if (need) {
-            const uint32_t idx = wpos + __popc(mask & lt);
-            if (idx >= n_words) overrun = true;
-            x = (x << 16) | ring[idx & (kRingWords - 1)];
-        }
-        wpos += __popc(mask);
-        out[(rd << 5) + lane] = (uint8_t)e.x;
+    uint32_t wpos2 = 0, trigger2 = 2 * kRingChunk;
+    uint8_t *op = out + lane;
+    uint32_t rd = n >> 5;
+    // Refill: when the words of chunk j are consumed, chunk j+4 is requested into its place; the wait
+    // at the next firing has had >= 64 words of decoding to hide behind. Checked every 4 rounds
+    // (<= 128 words): with firings up to j-1 done, chunks up to j+2 have landed, which covers
+    // every word below trigger_j + 128 that the next 4 rounds can read.
+#define ACEAPEX_RING_REFILL()                                                                          \
+    while (wpos2 >= trigger2) {                                                                        \
+        cp_async_wait_all();                                                                           \
+        __syncwarp();                                                                                  \
+        const uint32_t boff_ = trigger2 + 6 * kRingChunk + 4 * lane;   /* chunk trigger/64 + 3 */      \
+        if (boff_ < wbytes) cp_async4(ws.ring + (boff_ & (2 * kRingWords - 1)), words_sec + boff_);   \
+        cp_async_commit();                                                                             \
+        trigger2 += 2 * kRingChunk;                                                                    \
+    }
+    for (; rd >= 4; rd -= 4) {
+        ACEAPEX_RING_REFILL();
+        uint32_t s0, s1, s2, s3;
+        ACEAPEX_RANS_ROUND(s0);
+        ACEAPEX_RANS_ROUND(s1);
+        ACEAPEX_RANS_ROUND(s2);
+        ACEAPEX_RANS_ROUND(s3);
+        op[0] = (uint8_t)s0;
+        op[32] = (uint8_t)s1;
+        op[64] = (uint8_t)s2;
+        op[96] = (uint8_t)s3;
+        op += 128;
+    }
+    ACEAPEX_RING_REFILL();
+    for (; rd; rd--) {
+        uint32_t s0;
+        ACEAPEX_RANS_ROUND(s0);
+        op[0] = (uint8_t)s0;
+        op += 32;
     }
     if (n & 31u) {                                                   // ragged last round
-        if (wpos >= trigger) { cp_async_wait_all(); __syncwarp(); }
+        ACEAPEX_RING_REFILL();
         const bool active = lane < (n & 31u);
-        bool need = false;
-        uint32_t sym = 0;
-        if (active) {
-            const uint32_t slot = x & (kM - 1);
-            const uint2 e = syml[t8[slot]];
-            sym = e.x;
-            x = e.y * (x >> kProbBits) + (slot + (uint32_t)((int32_t)e.x >> 8));
-            need = x < kRansL;
+        const uint32_t x_keep = x;
+        uint32_t s0;
+        {
+            const uint32_t slot_ = x & (kM - 1);
+            const uint32_t i_ = lds_u8(slot_ | ws.a_t8);
+            const uint2 e_ = lds_v2(i_ * 8u + ws.a_syml);
+            x = e_.y * (x >> kProbBits) + (slot_ + (uint32_t)((int32_t)e_.x >> 8));
+            const bool need_ = active && x < kRansL;
+            const uint32_t mask_ = __ballot_sync(0xFFFFFFFFu, need_);
+            const uint32_t w_ = lds_u16(((wpos2 + 2u * __popc(mask_ & lt)) & (2 * kRingWords - 1)) | ws.a_ring);
+            if (need_) x = (x << 16) | w_;
+            wpos2 += 2u * __popc(mask_);
+            s0 = e_.x;
         }
-        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, need);
-        if (need) {
-            const uint32_t idx = wpos + __popc(mask & lt);
-            if (idx >= n_words) overrun = true;
-            x = (x << 16) | ring[idx & (kRingWords - 1)];
-        }
-        wpos += __popc(mask);
-        if (active) out[(full << 5) + lane] = (uint8_t)sym;
+        if (active) op[0] = (uint8_t)s0; else x = x_keep;
     }
+#undef ACEAPEX_RING_REFILL
     cp_async_wait_all();
-    const bool good = !overrun && x == kRansL;
-    return __all_sync(0xFFFFFFFFu, good) && wpos == n_words;
+    return __all_sync(0xFFFFFFFFu, x == kRansL) && wpos2 == wbytes;
 }
 
 // Kernel: every warp takes (block, stream) units from a counter until none is left.
 //   list != nullptr: the blocks are list[0 .. min(*n_list, max_slots)) (isolated path);
 //   else:            the blocks are first .. first+count-1.
-// Unit u -> block index u/3 (= slot), stream u%3. Output: the slot's LIT/LEN/OFF areas.
+// Unit u -> stream u / nb in the order LIT, OFF, LEN; block index u % nb (= slot). Output: the slot's areas.
 __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, SlotLayout sl, uint8_t *slots, const uint64_t *list,
                                                  const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                                                  uint32_t count, Control *ctl)
 {
-    extern __shared__ __align__(16) uint8_t smem_entropy[];
+    extern __shared__ __align__(1024) uint8_t smem_entropy[];
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-    uint8_t *wsm = smem_entropy + warp * kEntropyWarpSmem;
+    WarpSmem ws;
+    {
+        const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(smem_entropy);
+        const uint32_t pad = (0u - a0) & (kT8Bytes - 1);              // t8 region 4096-aligned in the shared window
+        uint8_t *base = smem_entropy + pad;
+        ws.t8 = base + warp * kT8Bytes;
+        ws.syml = reinterpret_cast<uint2 *>(base + kEntropyWarps * kT8Bytes + warp * kSymlBytes);
+        ws.ring = base + kEntropyWarps * (kT8Bytes + kSymlBytes) + warp * kRingBytes;
+        ws.a_t8 = (uint32_t)__cvta_generic_to_shared(ws.t8);
+        ws.a_syml = (uint32_t)__cvta_generic_to_shared(ws.syml);
+        ws.a_ring = (uint32_t)__cvta_generic_to_shared(ws.ring);
+    }
     uint32_t nb = count;
     if (list) { nb = *n_list; if (nb > max_slots) nb = max_slots; }
     const uint32_t n_units = 3 * nb;
@@ -216,8 +276,9 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, Sl
         if (lane == 0) u = atomicAdd(&ctl->unit, 1u);
         u = __shfl_sync(0xFFFFFFFFu, u, 0);
         if (u >= n_units) break;
-        const uint32_t bi = u / 3;
-        const int s = (int)(u - 3 * bi);
+        // longest first: all LIT streams, then OFF, then LEN (balances the tail of the launch)
+        const uint32_t so = u / nb, bi = u - so * nb;
+        const int s = so == 0 ? LIT : (so == 1 ? OFF : LEN);
         const uint64_t blk = list ? list[bi] : first + bi;
         uint8_t *slot = slots + (size_t)bi * sl.stride;
         SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
@@ -238,7 +299,7 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, Sl
             const uint32_t tb = s == LIT ? r.tbl_bytes[LIT] : (s == LEN ? r.tbl_bytes[LEN] : r.tbl_bytes[OFF]);
             const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
             const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
-            ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, wsm, lane);
+            ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
             if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
         } else if (lane == 0) {
             raise(ctl, kStRecord, blk);
