@@ -91,7 +91,7 @@ inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
 }
 
 inline size_t entropy_smem() { return kEntropySmem; }
-inline size_t match_smem(const SlotLayout &sl) { return kB + 3072 + 15 * (size_t)sl.ms + 64; }
+inline size_t match_smem(const SlotLayout &sl) { return match_smem_bytes(sl.ms); }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                    uint32_t count, cudaStream_t st)
@@ -280,7 +280,7 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         c->epoch = 1;
     }
     if (cudaMemsetAsync(&c->sc.ctl->watermark, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-    const uint32_t aligned = ((uintptr_t)d_out & 15) == 0;
+    const uint32_t aligned = ((uintptr_t)d_out & 3) == 0;
     for (uint64_t first = 0; first < c->cv.n_blocks; first += c->sc.n_slots) {
         const uint64_t rest = c->cv.n_blocks - first;
         const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);

@@ -160,50 +160,84 @@ __device__ inline unsigned long long advance_watermark(Control *ctl, const uint3
     return w;
 }
 
-// Source byte of a match at absolute position p: inside the block from the tile, else from the
-// output buffer (an earlier, completed block).
-__device__ inline uint32_t src_byte(const uint8_t *tile, const uint8_t *out, uint64_t B0, uint64_t p)
+// ---- decode_all match kernel --------------------------------------------------------------------
+//
+// Output-centric and branch-free. After the parse every output byte belongs to exactly one *run*:
+// the literal run of sequence q (run index 2q+1), the match of sequence q (2q+2) or the trailing
+// literals (2n+1). Two bitmaps over the 16,384 output offsets mark where sequences start (S) and
+// where matches start (D); the run that owns offset o is
+//     r(o) = #S bits <= o  +  #D bits <= o          (a rank word + two popcounts, no search)
+// and its source byte sits at address delta[r] + o, where delta[r] is
+//     literal run: &LIT[litpos_q] - start_q          (decoded LIT stream in the slot)
+//     match:       &out[src_q]   - dst_q             (absolute offset into the output buffer)
+// so literals and copies are the same instruction sequence: one 8-byte table load and one byte load
+// per output byte, four bytes per thread per step, one 32-bit store straight to the output buffer
+// (no staging tile: in-block sources are read back from the output buffer as well, which gives
+// cross-block and in-block copies one address space).
+//
+// Matches with tag >= 1 (source range reaches into this block, FORMAT.md section 4) are produced
+// by pass 0 with whatever the buffer held and then rewritten level by level from a list sorted by tag.
+
+constexpr uint32_t kMatchFixedSmem = 4096 + 1024;   // bm2 + rk
+
+__host__ __device__ inline uint32_t match_smem_bytes(uint32_t ms) { return kMatchFixedSmem + 8 * ms + 16 * ms + 16; }
+
+__device__ inline uint32_t ldg_u8(unsigned long long a)
 {
-    return p >= B0 ? tile[p - B0] : out[p];
+    uint32_t v;
+    asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(a) : "memory");
+    return v;
 }
 
-// decode_all, match layer. One CTA per block; block ids are handed out in increasing order by a
-// ticket, so a CTA only ever waits for blocks whose CTAs are already running or finished.
-//   slots: decoded streams of blocks first .. first+count-1 (slot i = block first+i).
-//
-// Pass 0 is output-centric: every thread produces groups of 4 consecutive output bytes. The
-// sequence that owns output offset o is rank[o>>5] + popc(bitmap word below o) - 1, where the
-// bitmap marks the start offset of every sequence: no search. Literal bytes come from the LIT
-// stream, bytes of tag-0 matches (source entirely in earlier blocks) from the output buffer.
-// Matches with tag >= 1 (source inside this block) follow level by level (FORMAT.md section 4).
+// Exclusive prefix sums of two values per thread over the CTA.
+__device__ inline void block_excl_scan2(uint32_t a, uint32_t b, uint32_t (*ws)[2] /* [kMatchWarps] smem */,
+                                        uint32_t &ea, uint32_t &eb, uint32_t &ta, uint32_t &tb)
+{
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    uint32_t wa, wb;
+    const uint32_t ia = warp_excl_scan(a, lane, wa), ib = warp_excl_scan(b, lane, wb);
+    __syncthreads();
+    if (lane == 0) { ws[warp][0] = wa; ws[warp][1] = wb; }
+    __syncthreads();
+    uint32_t ba = 0, bb = 0, sa = 0, sb = 0;
+#pragma unroll
+    for (uint32_t w = 0; w < kMatchWarps; w++) {
+        const uint32_t xa = ws[w][0], xb = ws[w][1];
+        if (w < warp) { ba += xa; bb += xb; }
+        sa += xa; sb += xb;
+    }
+    ea = ba + ia; eb = bb + ib; ta = sa; tb = sb;
+}
+
 __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayout sl, const uint8_t *slots,
                                                           uint64_t first, uint32_t count, uint8_t *out,
-                                                          uint32_t out_aligned16, Control *ctl, uint32_t *done,
+                                                          uint32_t out_aligned4, Control *ctl, uint32_t *done,
                                                           uint32_t epoch)
 {
     extern __shared__ __align__(16) uint8_t smem[];
-    __shared__ uint32_t warp_sums[kMatchWarps + 1];
-    __shared__ uint32_t s_ticket;
+    __shared__ uint32_t ws2[kMatchWarps][2];
+    __shared__ uint32_t s_ticket, s_ntag, s_bad;
     __shared__ unsigned long long s_below;
-    __shared__ uint32_t s_maxtag;
+    __shared__ uint32_t s_cnt[16], s_cur[16];
 
-    uint8_t *tile = smem;                                    // 16384
-    uint32_t *bm = reinterpret_cast<uint32_t *>(smem + kB);  // 512 words
-    uint16_t *rank = reinterpret_cast<uint16_t *>(smem + kB + 2048);   // 512
-    Tokens t;
-    t.src = reinterpret_cast<uint64_t *>(smem + kB + 3072);
-    t.start = reinterpret_cast<uint16_t *>(smem + kB + 3072 + 8 * sl.ms);
-    t.dst = t.start + (sl.ms + 16);
-    t.litpos = t.dst + sl.ms;
-    t.bm = bm;
-    uint8_t *tags = reinterpret_cast<uint8_t *>(t.litpos + (sl.ms + 16));   // [ms]
+    const uint32_t ms = sl.ms;
+    uint2 *bm2 = reinterpret_cast<uint2 *>(smem);                                   // [512] {S word, D word}
+    uint16_t *rk = reinterpret_cast<uint16_t *>(smem + 4096);                       // [512]
+    uint16_t *tlist = reinterpret_cast<uint16_t *>(smem + kMatchFixedSmem);         // [ms] k | tag << 12, unsorted
+    uint16_t *slist = tlist + ms;                                                   // [ms] sorted by tag
+    uint16_t *dstv = slist + ms;                                                    // [ms]
+    uint16_t *mlen = dstv + ms;                                                     // [ms]
+    unsigned long long *delta = reinterpret_cast<unsigned long long *>(smem + kMatchFixedSmem + 8 * ms);   // [2*ms+2]
 
-    if (threadIdx.x == 0) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    if (tid == 0) {
         s_ticket = atomicAdd(&ctl->ticket, 1u);
         s_below = 0;
-        s_maxtag = 0;
+        s_ntag = 0;
+        s_bad = 0;
     }
-    for (uint32_t i = threadIdx.x; i < 512; i += kMatchThreads) bm[i] = 0;
+    if (tid < 16) s_cnt[tid] = 0;
+    reinterpret_cast<uint4 *>(bm2)[tid] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     const uint32_t bi = s_ticket;
     if (bi < count) {
@@ -212,108 +246,181 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         const uint8_t *slot = slots + (size_t)bi * sl.stride;
         const SlotHdr *hdr = reinterpret_cast<const SlotHdr *>(slot + sl.o_hdr);
         const Record r = open_record(cv, blk);
-        bool ok = r.ok && !(hdr->bad[0] | hdr->bad[1] | hdr->bad[2]) && r.n_seq <= sl.ms;
+        bool ok = r.ok && !(hdr->bad[0] | hdr->bad[1] | hdr->bad[2]) && r.n_seq <= ms;
+        const uint32_t n = r.n_seq, blen = r.block_len;
+        uint32_t ll_total = 0, all_total = 0;
         if (ok) {
-            ok = parse_tokens(r, blk, slot + sl.o_len, slot + sl.o_off, t, warp_sums, (uint64_t *)&s_below);
-            if (!ok && threadIdx.x == 0) raise(ctl, kStTokens, blk);
+            // ---- parse (FORMAT.md section 4): thread t owns sequences [k0, k1)
+            const uint32_t per = (n + kMatchThreads - 1) / kMatchThreads;
+            const uint32_t k0 = min(n, tid * per), k1 = min(n, k0 + per);
+            const uint16_t *len16 = reinterpret_cast<const uint16_t *>(slot + sl.o_len);
+            const uint8_t *off_s = slot + sl.o_off;
+            const uint16_t *extras = reinterpret_cast<const uint16_t *>(r.rec + r.extras_off);
+            const uint8_t *tagsec = r.rec + r.tags_off;
+            uint32_t esc = 0, sum_ll = 0, sum_all = 0;
+            for (uint32_t k = k0; k < k1; k++) {
+                const uint32_t v = len16[k], ll = v & 0xFFu, ml = v >> 8;
+                esc += (ll == 255) + (ml == 255);
+                sum_ll += ll;
+                sum_all += ll + ml + 4;
+            }
+            uint32_t esc_base = 0, esc_total;
+            if (r.n_extras == 0) {
+                esc_total = __syncthreads_or(esc != 0) ? 1u : 0u;     // any escape without extras is invalid
+            } else {
+                uint32_t d0, d1;
+                block_excl_scan2(esc, 0, ws2, esc_base, d0, esc_total, d1);
+                if (esc_total == r.n_extras && esc) {                 // redo the sums with the true values
+                    uint32_t e = esc_base;
+                    sum_ll = sum_all = 0;
+                    for (uint32_t k = k0; k < k1; k++) {
+                        const uint32_t v = len16[k];
+                        uint32_t ll = v & 0xFFu, ml = v >> 8;
+                        if (ll == 255) ll = extras[e++];
+                        if (ml == 255) ml = extras[e++];
+                        sum_ll += ll;
+                        sum_all += ll + ml + 4;
+                    }
+                }
+            }
+            ok = esc_total == r.n_extras;                              // CTA-uniform
+            uint32_t ll_base = 0, all_base = 0;
+            if (ok) {
+                block_excl_scan2(sum_ll, sum_all, ws2, ll_base, all_base, ll_total, all_total);
+                ok = ll_total <= r.n_lit && all_total + (r.n_lit - ll_total) == blen;
+            }
+            if (ok) {
+                const unsigned long long lit_a = (unsigned long long)__cvta_generic_to_global(slot + sl.o_lit);
+                const unsigned long long out_a = (unsigned long long)__cvta_generic_to_global(out);
+                bool bad = false;
+                uint64_t below = 0;                                    // 1 + highest earlier block read
+                uint32_t e = esc_base, lp = ll_base, pos = all_base;
+                const uint32_t onb = r.off_nbytes;
+                for (uint32_t k = k0; k < k1; k++) {
+                    const uint32_t v = len16[k];
+                    uint32_t ll = v & 0xFFu, ml = v >> 8;
+                    if (ll == 255) ll = extras[e++];
+                    if (ml == 255) ml = extras[e++];
+                    ml += 4;
+                    uint64_t src = 0;
+                    for (uint32_t j = 0; j < onb; j++) src |= (uint64_t)off_s[k * onb + j] << (8 * j);
+                    const uint32_t tg = (tagsec[k >> 1] >> ((k & 1) * 4)) & 15u;
+                    // pos <= all_total <= 16384 holds for every sequence once the sums were accepted
+                    if (pos < kB) atomicOr(&bm2[pos >> 5].x, 1u << (pos & 31));
+                    delta[2 * k + 1] = lit_a + lp - pos;
+                    pos += ll; lp += ll;
+                    if (pos < kB) atomicOr(&bm2[pos >> 5].y, 1u << (pos & 31));
+                    delta[2 * k + 2] = out_a + src - pos;
+                    dstv[k] = (uint16_t)pos;
+                    mlen[k] = (uint16_t)ml;
+                    if (src + ml > B0 + pos) bad = true;               // strictly before, non-overlapping
+                    if (src < B0) {
+                        const uint64_t last = (src + ml < B0 ? src + ml : B0) - 1;
+                        const uint64_t need = (last >> kBlockLog2) + 1;
+                        if (need > below) below = need;
+                    }
+                    if (tg) {
+                        tlist[atomicAdd(&s_ntag, 1u)] = (uint16_t)(k | tg << 12);
+                        atomicAdd(&s_cnt[tg], 1u);
+                    }
+                    pos += ml;
+                }
+                if (tid == kMatchThreads - 1) {                        // trailing literals: run 2n+1
+                    if (all_total < blen) atomicOr(&bm2[all_total >> 5].x, 1u << (all_total & 31));
+                    delta[2 * n + 1] = lit_a + ll_total - all_total;
+                }
+                if (below) atomicMax(&s_below, (unsigned long long)below);
+                if (bad) s_bad = 1;
+            }
+            __syncthreads();
+            ok = ok && !s_bad;
+            if (!ok && tid == 0) raise(ctl, kStTokens, blk);
+        } else if (tid == 0 && !r.ok) {
+            raise(ctl, kStRecord, blk);
         }
         if (ok) {
-            const uint32_t n = r.n_seq, blen = r.block_len;
-            const uint8_t *lit = slot + sl.o_lit;
-            const uint8_t *tagsec = r.rec + r.tags_off;
-            uint32_t mt = 0;
-            for (uint32_t k = threadIdx.x; k < n; k += kMatchThreads) {
-                const uint32_t tg = (tagsec[k >> 1] >> ((k & 1) * 4)) & 15u;
-                tags[k] = (uint8_t)tg;
-                mt = max(mt, tg);
-            }
-            if (mt) atomicMax(&s_maxtag, mt);
-            // rank[w] = number of sequence starts in bitmap words before w
+            // rk[w] = number of S and D bits in the words before w; tag list sorted by level
             {
-                uint32_t p0 = 0, p1 = 0, p2 = 0, p3 = 0;
-                if (threadIdx.x < 128) {
-                    const uint4 w = reinterpret_cast<const uint4 *>(bm)[threadIdx.x];
-                    p0 = __popc(w.x); p1 = __popc(w.y); p2 = __popc(w.z); p3 = __popc(w.w);
+                const uint4 w = reinterpret_cast<const uint4 *>(bm2)[tid];            // words 2*tid, 2*tid+1
+                const uint32_t p0 = __popc(w.x) + __popc(w.y), p1 = __popc(w.z) + __popc(w.w);
+                uint32_t r0, d0, t0, t1;
+                block_excl_scan2(p0 + p1, 0, ws2, r0, d0, t0, t1);
+                reinterpret_cast<uint32_t *>(rk)[tid] = r0 | (r0 + p0) << 16;
+            }
+            const uint32_t ntag = s_ntag;
+            if (ntag) {
+                if (tid == 0) {
+                    uint32_t acc = 0;
+                    for (int t = 0; t < 16; t++) { s_cur[t] = acc; acc += s_cnt[t]; s_cnt[t] = acc; }   // s_cnt[t] = end of level t
                 }
-                uint32_t tot;
-                const uint32_t r0 = block_excl_scan(p0 + p1 + p2 + p3, warp_sums, tot);
-                if (threadIdx.x < 128)
-                    reinterpret_cast<uint2 *>(rank)[threadIdx.x] =
-                        make_uint2(r0 | (r0 + p0) << 16, (r0 + p0 + p1) | (r0 + p0 + p1 + p2) << 16);
+                __syncthreads();
+                for (uint32_t i = tid; i < ntag; i += kMatchThreads) {
+                    const uint32_t e = tlist[i];
+                    slist[atomicAdd(&s_cur[e >> 12], 1u)] = (uint16_t)e;
+                }
             }
             // wait until every earlier block this block copies from is complete
-            const uint32_t warp = threadIdx.x >> 5;
-            const uint64_t below = s_below;                  // 1 + highest earlier block read
+            const uint64_t below = s_below;
             if (below && warp == 0) {
                 while (advance_watermark(ctl, done, cv.n_blocks, epoch) < below) __nanosleep(64);
                 __threadfence();
             }
             __syncthreads();
-            // pass 0: literals and tag-0 matches, 4 output bytes per thread per step
-            for (uint32_t o = 4 * threadIdx.x; o < blen; o += 4 * kMatchThreads) {
-                const uint32_t w = bm[o >> 5], sh = o & 31u;
-                const uint32_t q = (uint32_t)rank[o >> 5] + __popc(w & ((2u << sh) - 1u)) - 1u;
-                const uint32_t st = t.start[q], d = q < n ? t.dst[q] : blen;
-                uint32_t v = 0;
-                const bool one_seq = ((w >> sh) & 0xEu) == 0 && o + 4 <= blen;
-                if (one_seq && o + 4 <= d) {                 // four literal bytes of sequence q
-                    const uint8_t *p = lit + t.litpos[q] + (o - st);
-                    v = p[0] | p[1] << 8 | p[2] << 16 | p[3] << 24;
-                } else if (one_seq && o >= d) {              // four bytes of match q
-                    if (tags[q] == 0) {
-                        const uint8_t *p = out + t.src[q] + (o - d);
-                        v = p[0] | p[1] << 8 | p[2] << 16 | p[3] << 24;
-                    }
-                } else {                                     // a boundary inside the group
-                    uint32_t qq = q, s0 = st, dd = d;
-                    for (uint32_t j = 0; j < 4 && o + j < blen; j++) {
-                        const uint32_t oj = o + j;
-                        if (j && ((w >> (sh + j)) & 1u)) { qq++; s0 = oj; dd = qq < n ? t.dst[qq] : blen; }
-                        uint32_t b = 0;
-                        if (oj < dd) b = lit[t.litpos[qq] + (oj - s0)];
-                        else if (tags[qq] == 0) b = out[t.src[qq] + (oj - dd)];
-                        v |= b << (8 * j);
+            // ---- pass 0: every output byte from delta[r(o)] + o
+            const unsigned long long outB = (unsigned long long)__cvta_generic_to_global(out) + B0;
+            for (uint32_t o = 4 * tid; o + 4 <= blen; o += 4 * kMatchThreads) {
+                const uint2 w = bm2[o >> 5];
+                const uint32_t sh = o & 31u, m = (2u << sh) - 1u;
+                const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
+                const uint32_t t = w.x >> sh, u = w.y >> sh;
+                const uint32_t r1 = r0 + ((t >> 1) & 1u) + ((u >> 1) & 1u);
+                const uint32_t r2 = r1 + ((t >> 2) & 1u) + ((u >> 2) & 1u);
+                const uint32_t r3 = r2 + ((t >> 3) & 1u) + ((u >> 3) & 1u);
+                const uint32_t b0 = ldg_u8(delta[r0] + o);
+                const uint32_t b1 = ldg_u8(delta[r1] + o + 1);
+                const uint32_t b2 = ldg_u8(delta[r2] + o + 2);
+                const uint32_t b3 = ldg_u8(delta[r3] + o + 3);
+                if (out_aligned4) {
+                    *reinterpret_cast<uint32_t *>(outB + o) = b0 | b1 << 8 | b2 << 16 | b3 << 24;
+                } else {
+                    uint8_t *p = reinterpret_cast<uint8_t *>(outB + o);
+                    p[0] = (uint8_t)b0; p[1] = (uint8_t)b1; p[2] = (uint8_t)b2; p[3] = (uint8_t)b3;
+                }
+            }
+            if (tid < (blen & 3u)) {                                   // ragged tail of a short last block
+                const uint32_t o = (blen & ~3u) + tid;
+                const uint2 w = bm2[o >> 5];
+                const uint32_t m = (2u << (o & 31u)) - 1u;
+                const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
+                *reinterpret_cast<uint8_t *>(outB + o) = (uint8_t)ldg_u8(delta[r0] + o);
+            }
+            // ---- matches whose source reaches into this block, level by level, 8 lanes per match
+            if (ntag) {
+                for (uint32_t level = 1; level < 16; level++) {
+                    const uint32_t i0 = s_cnt[level - 1], i1 = s_cnt[level];
+                    if (i0 == i1) continue;                            // CTA-uniform
+                    __syncthreads();                                   // the previous level (or pass 0) is in place
+                    for (uint32_t i = i0 + (tid >> 3); i < i1; i += kMatchThreads / 8) {
+                        const uint32_t k = slist[i] & 0xFFFu;
+                        const uint32_t d = dstv[k], ml = mlen[k];
+                        const unsigned long long sp = delta[2 * k + 2] + d, dp = outB + d;
+                        for (uint32_t j = tid & 7u; j < ml; j += 8)
+                            *reinterpret_cast<uint8_t *>(dp + j) = (uint8_t)ldg_u8(sp + j);
                     }
                 }
-                *reinterpret_cast<uint32_t *>(tile + o) = v;
             }
-            __syncthreads();
-            // matches whose source lies (partly) inside this block, level by level
-            const uint32_t maxtag = s_maxtag;
-            for (uint32_t level = 1; level <= maxtag; level++) {
-                for (uint32_t k = threadIdx.x; k < n; k += kMatchThreads) {
-                    if (tags[k] != level) continue;
-                    const uint32_t d = t.dst[k], ml = t.start[k + 1] - d;
-                    const uint64_t src = t.src[k];
-                    for (uint32_t j = 0; j < ml; j++) tile[d + j] = (uint8_t)src_byte(tile, out, B0, src + j);
-                }
-                __syncthreads();
-            }
-            // tile -> output
-            uint8_t *dstp = out + B0;
-            if (out_aligned16) {
-                const uint32_t nvec = blen >> 4;
-                const uint4 *tv = reinterpret_cast<const uint4 *>(tile);
-                uint4 *ov = reinterpret_cast<uint4 *>(dstp);
-                for (uint32_t i = threadIdx.x; i < nvec; i += kMatchThreads) ov[i] = tv[i];
-                for (uint32_t i = (nvec << 4) + threadIdx.x; i < blen; i += kMatchThreads) dstp[i] = tile[i];
-            } else {
-                for (uint32_t i = threadIdx.x; i < blen; i += kMatchThreads) dstp[i] = tile[i];
-            }
-        } else if (threadIdx.x == 0 && !r.ok) {
-            raise(ctl, kStRecord, blk);
         }
         // publish (also for a bad block: later blocks must not wait forever)
         __threadfence();
         __syncthreads();
-        if (threadIdx.x < 32) {
-            if (threadIdx.x == 0) st_release_u32(done + blk, epoch);
+        if (tid < 32) {
+            if (tid == 0) st_release_u32(done + blk, epoch);
             __syncwarp();
             advance_watermark(ctl, done, cv.n_blocks, epoch);
         }
     }
     // last CTA out re-arms the ticket for the next launch
-    if (threadIdx.x == 0) {
+    if (tid == 0) {
         __threadfence();
         if (atomicAdd(&ctl->ticket_exit, 1u) == gridDim.x - 1) {
             ctl->ticket = 0;
