@@ -91,7 +91,7 @@ inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
 }
 
 inline size_t entropy_smem() { return kEntropySmem; }
-inline size_t match_smem(const SlotLayout &sl) { return match_smem_bytes(sl.ms); }
+inline size_t match_smem(const aceapex_ctx *c) { return match_smem_bytes(c->sl.ms, c->cv.W); }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                    uint32_t count, cudaStream_t st)
@@ -201,7 +201,7 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
     if (rc != ACEAPEX_OK) { aceapex_close(c); return rc; }
 
     c->sl = make_slot_layout(res.max_n_seq, c->cv.W);
-    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem(c->sl)) != cudaSuccess) {
+    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem(c)) != cudaSuccess) {
         aceapex_close(c);
         return ACEAPEX_E_CUDA;
     }
@@ -288,7 +288,7 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         if (rc != ACEAPEX_OK) return rc;
         {
             LaunchScope ls(c, K_MATCH, st);
-            k_match<<<count, kMatchThreads, match_smem(c->sl), st>>>(c->cv, c->sl, c->sc.slots, first, count,
+            k_match<<<count, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
                                                                     static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
                                                                     c->sc.done, c->epoch);
         }
@@ -451,6 +451,16 @@ int aceapex_profile_read(aceapex_ctx *c, uint64_t *launches, double *ms)
     c->prof_recs.clear();
     return rc;
 }
+
+#ifdef ACEAPEX_TRACE
+int aceapex_debug_trace(unsigned long long *out16, int reset)
+{
+    cudaDeviceSynchronize();
+    if (out16) cudaMemcpyFromSymbol(out16, g_trace, sizeof(unsigned long long) * 16);
+    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(g_trace, z, sizeof z); }
+    return 0;
+}
+#endif
 
 const char *aceapex_kernel_name(int id) { return id >= 0 && id < K_COUNT ? kKernelNames[id] : nullptr; }
 

@@ -133,31 +133,44 @@ __device__ inline void st_release_u32(uint32_t *p, uint32_t v)
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Advance the watermark over every leading block whose done flag carries this call's epoch.
-// Called by all 32 lanes of one warp: 32 flags are examined per round trip. Returns the new
-// watermark (warp-uniform). The flags were read with acquire semantics and the fence orders them
-// before the atomicMax, so whoever later acquires the watermark also sees those blocks' bytes.
-__device__ inline unsigned long long advance_watermark(Control *ctl, const uint32_t *done, uint64_t n_blocks,
-                                                       uint32_t epoch)
+// Publish block `blk` as complete and keep the watermark (number of leading complete blocks) moving.
+// Called by all 32 lanes of one warp after the block's bytes were fenced. Only the CTA that
+// completes the oldest outstanding block (watermark == blk) scans forward, 32 done flags per round
+// trip; everybody else sets its flag and leaves. The flag store and the watermark load, and on the
+// scanner's side the watermark store and the re-read of the next flag, are separated by
+// sequentially consistent fences (store-buffering pattern): whichever of the two CTAs comes second
+// sees the other's write, so the watermark never stalls below a completed block. Waiters acquire the
+// watermark; the scanner read the flags with acquire semantics and fenced before publishing it, so
+// a waiter also sees those blocks' bytes.
+__device__ inline void publish_block(Control *ctl, uint32_t *done, uint64_t n_blocks, uint32_t epoch, uint64_t blk)
 {
     const uint32_t lane = lane_id();
-    unsigned long long w0 = 0;
-    if (lane == 0) w0 = ld_acquire_u64(&ctl->watermark);
-    w0 = __shfl_sync(0xFFFFFFFFu, w0, 0);
-    unsigned long long w = w0;
-    for (;;) {
-        const unsigned long long idx = w + lane;
-        const bool f = idx < n_blocks && ld_acquire_u32(done + idx) == epoch;
-        const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
-        const uint32_t c = m == 0xFFFFFFFFu ? 32u : (uint32_t)__ffs(~m) - 1u;
-        w += c;
-        if (c < 32) break;
-    }
-    if (w > w0 && lane == 0) {
+    unsigned long long w = 0;
+    if (lane == 0) {
+        st_release_u32(done + blk, epoch);
         __threadfence();
-        atomicMax(&ctl->watermark, w);
+        w = ld_acquire_u64(&ctl->watermark);
     }
-    return w;
+    w = __shfl_sync(0xFFFFFFFFu, w, 0);
+    if (w != blk) return;
+    for (;;) {
+        for (;;) {
+            const unsigned long long idx = w + lane;
+            const bool f = idx < n_blocks && ld_acquire_u32(done + idx) == epoch;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
+            const uint32_t c = m == 0xFFFFFFFFu ? 32u : (uint32_t)__ffs(~m) - 1u;
+            w += c;
+            if (c < 32) break;
+        }
+        uint32_t again = 0;
+        if (lane == 0) {
+            __threadfence();
+            atomicMax(&ctl->watermark, w);
+            __threadfence();
+            again = w < n_blocks && ld_acquire_u32(done + w) == epoch;
+        }
+        if (!__shfl_sync(0xFFFFFFFFu, again, 0)) return;
+    }
 }
 
 // ---- decode_all match kernel --------------------------------------------------------------------
@@ -178,9 +191,23 @@ __device__ inline unsigned long long advance_watermark(Control *ctl, const uint3
 // Matches with tag >= 1 (source range reaches into this block, FORMAT.md section 4) are produced
 // by pass 0 with whatever the buffer held and then rewritten level by level from a list sorted by tag.
 
-constexpr uint32_t kMatchFixedSmem = 4096 + 1024;   // bm2 + rk
+#ifdef ACEAPEX_TRACE
+__device__ unsigned long long g_trace[16];
+#define TRACE_MARK(i) do { if (threadIdx.x == 0) { const long long t_ = clock64(); atomicAdd(&g_trace[i], (unsigned long long)(t_ - t_prev)); t_prev = t_; } } while (0)
+#define TRACE_DECL long long t_prev = clock64()
+#else
+#define TRACE_MARK(i) do { } while (0)
+#define TRACE_DECL do { } while (0)
+#endif
 
-__host__ __device__ inline uint32_t match_smem_bytes(uint32_t ms) { return kMatchFixedSmem + 8 * ms + 16 * ms + 16; }
+constexpr uint32_t kMatchFixedSmem = 4096 + 1024 + 16;   // bm2 + rk + delta[0] pad (delta[1] is 16-byte aligned)
+
+__host__ __device__ inline uint32_t match_smem_bytes(uint32_t ms, uint32_t W)
+{
+    // delta (16 ms + 16), dm (4 ms), tlist (2 ms), staged LEN / slist (2 ms), staged OFF (W ms + 16: the
+    // word-wise offset read may touch 11 bytes past the last offset), staged tags (ms / 2)
+    return kMatchFixedSmem + 16 * ms + 16 + 4 * ms + 2 * ms + 2 * ms + (W * ms + 16) + ms / 2;
+}
 
 __device__ inline uint32_t ldg_u8(unsigned long long a)
 {
@@ -209,27 +236,61 @@ __device__ inline void block_excl_scan2(uint32_t a, uint32_t b, uint32_t (*ws)[2
     ea = ba + ia; eb = bb + ib; ta = sa; tb = sb;
 }
 
+// The four source addresses of output bytes o .. o+3 (o a multiple of 4).
+struct Addr4 { unsigned long long a0, a1, a2, a3; };
+__device__ inline Addr4 run_addresses(const uint2 *bm2, const uint16_t *rk, const unsigned long long *delta, uint32_t o)
+{
+    const uint2 w = bm2[o >> 5];
+    const uint32_t sh = o & 31u, m = (2u << sh) - 1u;
+    const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
+    const uint32_t t = w.x >> sh, u = w.y >> sh;
+    const uint32_t r1 = r0 + ((t >> 1) & 1u) + ((u >> 1) & 1u);
+    const uint32_t r2 = r1 + ((t >> 2) & 1u) + ((u >> 2) & 1u);
+    const uint32_t r3 = r2 + ((t >> 3) & 1u) + ((u >> 3) & 1u);
+    Addr4 a;
+    a.a0 = delta[r0] + o;
+    a.a1 = delta[r1] + o + 1;
+    a.a2 = delta[r2] + o + 2;
+    a.a3 = delta[r3] + o + 3;
+    return a;
+}
+
+__device__ inline void store4(unsigned long long a, uint32_t v, uint32_t aligned4)
+{
+    if (aligned4) {
+        asm volatile("st.global.u32 [%0], %1;" ::"l"(a), "r"(v) : "memory");
+    } else {
+        asm volatile("st.global.u8 [%0], %1;" ::"l"(a), "r"(v) : "memory");
+        asm volatile("st.global.u8 [%0], %1;" ::"l"(a + 1), "r"(v >> 8) : "memory");
+        asm volatile("st.global.u8 [%0], %1;" ::"l"(a + 2), "r"(v >> 16) : "memory");
+        asm volatile("st.global.u8 [%0], %1;" ::"l"(a + 3), "r"(v >> 24) : "memory");
+    }
+}
+
 __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayout sl, const uint8_t *slots,
                                                           uint64_t first, uint32_t count, uint8_t *out,
                                                           uint32_t out_aligned4, Control *ctl, uint32_t *done,
                                                           uint32_t epoch)
 {
     extern __shared__ __align__(16) uint8_t smem[];
+    __shared__ uint32_t ws3[kMatchWarps][3];
     __shared__ uint32_t ws2[kMatchWarps][2];
-    __shared__ uint32_t s_ticket, s_ntag, s_bad;
-    __shared__ unsigned long long s_below;
+    __shared__ uint32_t s_ticket, s_ntag, s_bad, s_below;
     __shared__ uint32_t s_cnt[16], s_cur[16];
 
     const uint32_t ms = sl.ms;
     uint2 *bm2 = reinterpret_cast<uint2 *>(smem);                                   // [512] {S word, D word}
     uint16_t *rk = reinterpret_cast<uint16_t *>(smem + 4096);                       // [512]
-    uint16_t *tlist = reinterpret_cast<uint16_t *>(smem + kMatchFixedSmem);         // [ms] k | tag << 12, unsorted
-    uint16_t *slist = tlist + ms;                                                   // [ms] sorted by tag
-    uint16_t *dstv = slist + ms;                                                    // [ms]
-    uint16_t *mlen = dstv + ms;                                                     // [ms]
-    unsigned long long *delta = reinterpret_cast<unsigned long long *>(smem + kMatchFixedSmem + 8 * ms);   // [2*ms+2]
+    unsigned long long *delta = reinterpret_cast<unsigned long long *>(smem + 4096 + 1024 + 8);   // [2*ms+2]
+    uint32_t *dm = reinterpret_cast<uint32_t *>(smem + kMatchFixedSmem + 16 * ms + 16);          // [ms] dst | len << 16
+    uint16_t *tlist = reinterpret_cast<uint16_t *>(dm + ms);                        // [ms] k | tag << 12, unsorted
+    uint16_t *s_len16 = tlist + ms;                                                 // [ms] staged LEN stream (u8 pairs)
+    uint16_t *slist = s_len16;                                                      // [ms] tag list sorted by tag (after the parse)
+    uint8_t *s_off = reinterpret_cast<uint8_t *>(s_len16 + ms);                     // [W*ms] staged OFF stream
+    uint8_t *s_tags = s_off + cv.W * ms + 16;                                            // [ms/2] staged tag nibbles
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
     if (tid == 0) {
         s_ticket = atomicAdd(&ctl->ticket, 1u);
         s_below = 0;
@@ -237,9 +298,12 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         s_bad = 0;
     }
     if (tid < 16) s_cnt[tid] = 0;
-    reinterpret_cast<uint4 *>(bm2)[tid] = make_uint4(0, 0, 0, 0);
+    for (uint32_t i = tid; i < 256; i += kMatchThreads) reinterpret_cast<uint4 *>(bm2)[i] = make_uint4(0, 0, 0, 0);
+    unsigned long long wm_early = 0;                                   // thread 0: the watermark as of now (it only grows)
+    if (tid == 0) wm_early = ld_acquire_u64(&ctl->watermark);
     __syncthreads();
     const uint32_t bi = s_ticket;
+    TRACE_DECL;
     if (bi < count) {
         const uint64_t blk = first + bi;
         const uint64_t B0 = blk << kBlockLog2;
@@ -248,91 +312,152 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         const Record r = open_record(cv, blk);
         bool ok = r.ok && !(hdr->bad[0] | hdr->bad[1] | hdr->bad[2]) && r.n_seq <= ms;
         const uint32_t n = r.n_seq, blen = r.block_len;
-        uint32_t ll_total = 0, all_total = 0;
+        TRACE_MARK(0);
         if (ok) {
-            // ---- parse (FORMAT.md section 4): thread t owns sequences [k0, k1)
-            const uint32_t per = (n + kMatchThreads - 1) / kMatchThreads;
-            const uint32_t k0 = min(n, tid * per), k1 = min(n, k0 + per);
-            const uint16_t *len16 = reinterpret_cast<const uint16_t *>(slot + sl.o_len);
-            const uint8_t *off_s = slot + sl.o_off;
+            // ---- parse (FORMAT.md section 4). Warp w owns the sequences [w*cw, (w+1)*cw), lane-strided:
+            // in round i lane l holds sequence w*cw + 32*i + l, so loads coalesce and the prefix sums are
+            // one packed warp scan per round plus a carry.
+            const uint32_t cw = ((n + kMatchThreads - 1) / kMatchThreads) * 32;
+            const uint32_t wk0 = min(n, warp * cw), wk1 = min(n, wk0 + cw);
+            // Stage the decoded LEN / OFF streams and the tag nibbles into shared memory with one round of
+            // 16-byte async copies (sizes padded to 16 stay inside the slot areas / the record).
+            {
+                const uint32_t nl = (2 * n + 15) >> 4, no = (r.off_nbytes * n + 15) >> 4, nt = ((n + 1) / 2 + 15) >> 4;
+                const uint8_t *gl = slot + sl.o_len, *go = slot + sl.o_off, *gt = r.rec + r.tags_off;
+                for (uint32_t i = tid; i < nl; i += kMatchThreads) cp_async16(reinterpret_cast<uint8_t *>(s_len16) + 16 * i, gl + 16 * i);
+                for (uint32_t i = tid; i < no; i += kMatchThreads) cp_async16(s_off + 16 * i, go + 16 * i);
+                for (uint32_t i = tid; i < nt; i += kMatchThreads) cp_async16(s_tags + 16 * i, gt + 16 * i);
+                cp_async_commit();
+                cp_async_wait_all();
+                __syncthreads();
+            }
+            const uint16_t *len16 = s_len16;
+            const uint8_t *off_s = s_off;
             const uint16_t *extras = reinterpret_cast<const uint16_t *>(r.rec + r.extras_off);
-            const uint8_t *tagsec = r.rec + r.tags_off;
-            uint32_t esc = 0, sum_ll = 0, sum_all = 0;
-            for (uint32_t k = k0; k < k1; k++) {
-                const uint32_t v = len16[k], ll = v & 0xFFu, ml = v >> 8;
-                esc += (ll == 255) + (ml == 255);
-                sum_ll += ll;
-                sum_all += ll + ml + 4;
-            }
-            uint32_t esc_base = 0, esc_total;
-            if (r.n_extras == 0) {
-                esc_total = __syncthreads_or(esc != 0) ? 1u : 0u;     // any escape without extras is invalid
-            } else {
-                uint32_t d0, d1;
-                block_excl_scan2(esc, 0, ws2, esc_base, d0, esc_total, d1);
-                if (esc_total == r.n_extras && esc) {                 // redo the sums with the true values
-                    uint32_t e = esc_base;
-                    sum_ll = sum_all = 0;
-                    for (uint32_t k = k0; k < k1; k++) {
-                        const uint32_t v = len16[k];
-                        uint32_t ll = v & 0xFFu, ml = v >> 8;
-                        if (ll == 255) ll = extras[e++];
-                        if (ml == 255) ml = extras[e++];
-                        sum_ll += ll;
-                        sum_all += ll + ml + 4;
-                    }
+            const uint8_t *tagsec = s_tags;
+            const bool has_esc = r.n_extras != 0;                      // CTA-uniform
+            // A0 (only with escapes): escapes per warp -> extras base of each warp
+            uint32_t esc_base = 0;
+            if (has_esc) {
+                uint32_t esc = 0;
+                for (uint32_t k = wk0 + lane; k < wk1; k += 32) {
+                    const uint32_t v = len16[k];
+                    esc += ((v & 0xFFu) == 255) + ((v >> 8) == 255);
                 }
+                esc = __reduce_add_sync(0xFFFFFFFFu, esc);
+                if (lane == 0) ws3[warp][0] = esc;
+                __syncthreads();
+                uint32_t tot = 0;
+#pragma unroll
+                for (uint32_t w = 0; w < kMatchWarps; w++) { const uint32_t x = ws3[w][0]; if (w < warp) esc_base += x; tot += x; }
+                ok = tot == r.n_extras;
+                __syncthreads();
             }
-            ok = esc_total == r.n_extras;                              // CTA-uniform
-            uint32_t ll_base = 0, all_base = 0;
+            // A: sums per warp
+            uint32_t sum_ll = 0, sum_all = 0, any_esc = 0;
             if (ok) {
-                block_excl_scan2(sum_ll, sum_all, ws2, ll_base, all_base, ll_total, all_total);
-                ok = ll_total <= r.n_lit && all_total + (r.n_lit - ll_total) == blen;
+                uint32_t e_carry = esc_base;
+                for (uint32_t kb = wk0; kb < wk1; kb += 32) {
+                    const uint32_t k = kb + lane;
+                    uint32_t ll = 0, ml = 0;
+                    if (k < wk1) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
+                    const uint32_t e_ll = ll == 255, e_ml = ml == 259;
+                    any_esc |= e_ll | e_ml;
+                    if (has_esc) {
+                        uint32_t etot;
+                        uint32_t e = e_carry + warp_excl_scan(e_ll + e_ml, lane, etot);
+                        if (e_ll) ll = extras[e++];
+                        if (e_ml) ml = (uint32_t)extras[e] + 4;
+                        e_carry += etot;
+                    }
+                    sum_ll += ll;
+                    sum_all += ll + ml;
+                }
+                sum_ll = __reduce_add_sync(0xFFFFFFFFu, sum_ll);
+                sum_all = __reduce_add_sync(0xFFFFFFFFu, sum_all);
+                any_esc = __reduce_or_sync(0xFFFFFFFFu, any_esc);
+                if (lane == 0) { ws3[warp][0] = sum_ll; ws3[warp][1] = sum_all; ws3[warp][2] = any_esc; }
+            }
+            __syncthreads();
+            uint32_t ll_base = 0, all_base = 0, ll_total = 0, all_total = 0;
+            if (ok) {
+                uint32_t esc_seen = 0;
+#pragma unroll
+                for (uint32_t w = 0; w < kMatchWarps; w++) {
+                    const uint32_t xa = ws3[w][0], xb = ws3[w][1];
+                    if (w < warp) { ll_base += xa; all_base += xb; }
+                    ll_total += xa; all_total += xb; esc_seen |= ws3[w][2];
+                }
+                ok = ll_total <= r.n_lit && all_total + (r.n_lit - ll_total) == blen && (has_esc || !esc_seen);
             }
             if (ok) {
+                // B: positions, run table, bitmaps, tag list. Every partial sum is <= 16384 now.
                 const unsigned long long lit_a = (unsigned long long)__cvta_generic_to_global(slot + sl.o_lit);
                 const unsigned long long out_a = (unsigned long long)__cvta_generic_to_global(out);
+                const uint32_t onb = r.off_nbytes;                     // 1..8
+                const uint64_t src_mask = ~0ull >> (64 - 8 * onb);
                 bool bad = false;
-                uint64_t below = 0;                                    // 1 + highest earlier block read
-                uint32_t e = esc_base, lp = ll_base, pos = all_base;
-                const uint32_t onb = r.off_nbytes;
-                for (uint32_t k = k0; k < k1; k++) {
-                    const uint32_t v = len16[k];
-                    uint32_t ll = v & 0xFFu, ml = v >> 8;
-                    if (ll == 255) ll = extras[e++];
-                    if (ml == 255) ml = extras[e++];
-                    ml += 4;
-                    uint64_t src = 0;
-                    for (uint32_t j = 0; j < onb; j++) src |= (uint64_t)off_s[k * onb + j] << (8 * j);
-                    const uint32_t tg = (tagsec[k >> 1] >> ((k & 1) * 4)) & 15u;
-                    // pos <= all_total <= 16384 holds for every sequence once the sums were accepted
-                    if (pos < kB) atomicOr(&bm2[pos >> 5].x, 1u << (pos & 31));
-                    delta[2 * k + 1] = lit_a + lp - pos;
-                    pos += ll; lp += ll;
-                    if (pos < kB) atomicOr(&bm2[pos >> 5].y, 1u << (pos & 31));
-                    delta[2 * k + 2] = out_a + src - pos;
-                    dstv[k] = (uint16_t)pos;
-                    mlen[k] = (uint16_t)ml;
-                    if (src + ml > B0 + pos) bad = true;               // strictly before, non-overlapping
-                    if (src < B0) {
-                        const uint64_t last = (src + ml < B0 ? src + ml : B0) - 1;
-                        const uint64_t need = (last >> kBlockLog2) + 1;
-                        if (need > below) below = need;
+                uint64_t mx = 0;                                       // max end of a source range that starts below B0
+                uint32_t e_carry = esc_base, lp_carry = ll_base, pos_carry = all_base;
+                for (uint32_t kb = wk0; kb < wk1; kb += 32) {
+                    const uint32_t k = kb + lane;
+                    const bool act = k < wk1;
+                    uint32_t ll = 0, ml = 0;
+                    if (act) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
+                    if (has_esc) {
+                        const uint32_t e_ll = ll == 255, e_ml = ml == 259;
+                        uint32_t etot;
+                        uint32_t e = e_carry + warp_excl_scan(e_ll + e_ml, lane, etot);
+                        if (e_ll) ll = extras[e++];
+                        if (e_ml) ml = (uint32_t)extras[e] + 4;
+                        e_carry += etot;
                     }
-                    if (tg) {
-                        tlist[atomicAdd(&s_ntag, 1u)] = (uint16_t)(k | tg << 12);
-                        atomicAdd(&s_cnt[tg], 1u);
+                    uint32_t ptot;
+                    const uint32_t pre = warp_excl_scan(ll | (ll + ml) << 16, lane, ptot);
+                    const uint32_t lp = lp_carry + (pre & 0xFFFFu);    // first literal of sequence k
+                    const uint32_t st = pos_carry + (pre >> 16);       // in-block offset where sequence k starts
+                    const uint32_t d = st + ll;                        // ... and where its match starts
+                    lp_carry += ptot & 0xFFFFu;
+                    pos_carry += ptot >> 16;
+                    uint32_t tg = 0;
+                    if (act) {
+                        // src = the onb bytes at off_s[k * onb]: three aligned words, funnel-shifted and masked
+                        const uint32_t p = k * onb, sh = (p & 3u) * 8;
+                        const uint32_t *wp = reinterpret_cast<const uint32_t *>(off_s + (p & ~3u));
+                        const uint32_t w0 = wp[0], w1 = wp[1], w2 = wp[2];
+                        const uint32_t lo = __funnelshift_r(w0, w1, sh), hi = __funnelshift_r(w1, w2, sh);
+                        const uint64_t src = (((uint64_t)hi << 32) | lo) & src_mask;
+                        tg = (tagsec[k >> 1] >> ((k & 1) * 4)) & 15u;
+                        if (st < kB) atomicOr(&bm2[st >> 5].x, 1u << (st & 31));
+                        if (d < kB) atomicOr(&bm2[d >> 5].y, 1u << (d & 31));
+                        *reinterpret_cast<ulonglong2 *>(&delta[2 * k + 1]) = make_ulonglong2(lit_a + lp - st, out_a + src - d);
+                        dm[k] = d | ml << 16;
+                        if (src + ml > B0 + d) bad = true;             // strictly before, non-overlapping
+                        if (src < B0 && src + ml > mx) mx = src + ml;
                     }
-                    pos += ml;
+                    const uint32_t tm = __ballot_sync(0xFFFFFFFFu, tg != 0);
+                    if (tm) {                                          // warp-aggregated append to the tag list
+                        uint32_t tb = 0;
+                        if (lane == 0) tb = atomicAdd(&s_ntag, (uint32_t)__popc(tm));
+                        tb = __shfl_sync(0xFFFFFFFFu, tb, 0);
+                        if (tg) {
+                            tlist[tb + __popc(tm & lt)] = (uint16_t)(k | tg << 12);
+                            atomicAdd(&s_cnt[tg], 1u);
+                        }
+                    }
                 }
                 if (tid == kMatchThreads - 1) {                        // trailing literals: run 2n+1
                     if (all_total < blen) atomicOr(&bm2[all_total >> 5].x, 1u << (all_total & 31));
                     delta[2 * n + 1] = lit_a + ll_total - all_total;
                 }
-                if (below) atomicMax(&s_below, (unsigned long long)below);
-                if (bad) s_bad = 1;
+                uint32_t below = 0;                                    // 1 + highest earlier block read
+                if (mx) below = (uint32_t)(((mx < B0 ? mx : B0) - 1) >> kBlockLog2) + 1;
+                below = __reduce_max_sync(0xFFFFFFFFu, below);
+                if (lane == 0 && below) atomicMax(&s_below, below);
+                if (__any_sync(0xFFFFFFFFu, bad) && lane == 0) s_bad = 1;
             }
             __syncthreads();
+            TRACE_MARK(1);
             ok = ok && !s_bad;
             if (!ok && tid == 0) raise(ctl, kStTokens, blk);
         } else if (tid == 0 && !r.ok) {
@@ -341,11 +466,14 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         if (ok) {
             // rk[w] = number of S and D bits in the words before w; tag list sorted by level
             {
-                const uint4 w = reinterpret_cast<const uint4 *>(bm2)[tid];            // words 2*tid, 2*tid+1
-                const uint32_t p0 = __popc(w.x) + __popc(w.y), p1 = __popc(w.z) + __popc(w.w);
+                uint32_t p0 = 0, p1 = 0;
+                if (tid < 256) {
+                    const uint4 w = reinterpret_cast<const uint4 *>(bm2)[tid];        // words 2*tid, 2*tid+1
+                    p0 = __popc(w.x) + __popc(w.y); p1 = __popc(w.z) + __popc(w.w);
+                }
                 uint32_t r0, d0, t0, t1;
                 block_excl_scan2(p0 + p1, 0, ws2, r0, d0, t0, t1);
-                reinterpret_cast<uint32_t *>(rk)[tid] = r0 | (r0 + p0) << 16;
+                if (tid < 256) reinterpret_cast<uint32_t *>(rk)[tid] = r0 | (r0 + p0) << 16;
             }
             const uint32_t ntag = s_ntag;
             if (ntag) {
@@ -361,31 +489,32 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             }
             // wait until every earlier block this block copies from is complete
             const uint64_t below = s_below;
-            if (below && warp == 0) {
-                while (advance_watermark(ctl, done, cv.n_blocks, epoch) < below) __nanosleep(64);
-                __threadfence();
+            TRACE_MARK(2);
+            if (tid == 0) {
+                while (wm_early < below) { __nanosleep(100); wm_early = ld_acquire_u64(&ctl->watermark); }
             }
             __syncthreads();
-            // ---- pass 0: every output byte from delta[r(o)] + o
+            TRACE_MARK(3);
+            // ---- pass 0: every output byte from delta[r(o)] + o; 16 byte loads in flight per thread
             const unsigned long long outB = (unsigned long long)__cvta_generic_to_global(out) + B0;
-            for (uint32_t o = 4 * tid; o + 4 <= blen; o += 4 * kMatchThreads) {
-                const uint2 w = bm2[o >> 5];
-                const uint32_t sh = o & 31u, m = (2u << sh) - 1u;
-                const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
-                const uint32_t t = w.x >> sh, u = w.y >> sh;
-                const uint32_t r1 = r0 + ((t >> 1) & 1u) + ((u >> 1) & 1u);
-                const uint32_t r2 = r1 + ((t >> 2) & 1u) + ((u >> 2) & 1u);
-                const uint32_t r3 = r2 + ((t >> 3) & 1u) + ((u >> 3) & 1u);
-                const uint32_t b0 = ldg_u8(delta[r0] + o);
-                const uint32_t b1 = ldg_u8(delta[r1] + o + 1);
-                const uint32_t b2 = ldg_u8(delta[r2] + o + 2);
-                const uint32_t b3 = ldg_u8(delta[r3] + o + 3);
-                if (out_aligned4) {
-                    *reinterpret_cast<uint32_t *>(outB + o) = b0 | b1 << 8 | b2 << 16 | b3 << 24;
-                } else {
-                    uint8_t *p = reinterpret_cast<uint8_t *>(outB + o);
-                    p[0] = (uint8_t)b0; p[1] = (uint8_t)b1; p[2] = (uint8_t)b2; p[3] = (uint8_t)b3;
+            uint32_t ob = 4 * tid;
+            for (; ob + 12 * kMatchThreads + 4 <= blen; ob += 16 * kMatchThreads) {
+                Addr4 a[4];
+                uint32_t b[4][4];
+#pragma unroll
+                for (int u = 0; u < 4; u++) a[u] = run_addresses(bm2, rk, delta, ob + u * 4 * kMatchThreads);
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    b[u][0] = ldg_u8(a[u].a0); b[u][1] = ldg_u8(a[u].a1); b[u][2] = ldg_u8(a[u].a2); b[u][3] = ldg_u8(a[u].a3);
                 }
+#pragma unroll
+                for (int u = 0; u < 4; u++)
+                    store4(outB + ob + u * 4 * kMatchThreads, b[u][0] | b[u][1] << 8 | b[u][2] << 16 | b[u][3] << 24, out_aligned4);
+            }
+            for (; ob + 4 <= blen; ob += 4 * kMatchThreads) {
+                const Addr4 a = run_addresses(bm2, rk, delta, ob);
+                const uint32_t b0 = ldg_u8(a.a0), b1 = ldg_u8(a.a1), b2 = ldg_u8(a.a2), b3 = ldg_u8(a.a3);
+                store4(outB + ob, b0 | b1 << 8 | b2 << 16 | b3 << 24, out_aligned4);
             }
             if (tid < (blen & 3u)) {                                   // ragged tail of a short last block
                 const uint32_t o = (blen & ~3u) + tid;
@@ -394,30 +523,34 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
                 *reinterpret_cast<uint8_t *>(outB + o) = (uint8_t)ldg_u8(delta[r0] + o);
             }
+            __syncthreads();
+            TRACE_MARK(4);
             // ---- matches whose source reaches into this block, level by level, 8 lanes per match
             if (ntag) {
-                for (uint32_t level = 1; level < 16; level++) {
-                    const uint32_t i0 = s_cnt[level - 1], i1 = s_cnt[level];
+                uint32_t i0 = 0;
+                for (uint32_t level = 1; level < 16 && i0 < ntag; level++) {
+                    const uint32_t i1 = s_cnt[level];
                     if (i0 == i1) continue;                            // CTA-uniform
                     __syncthreads();                                   // the previous level (or pass 0) is in place
                     for (uint32_t i = i0 + (tid >> 3); i < i1; i += kMatchThreads / 8) {
                         const uint32_t k = slist[i] & 0xFFFu;
-                        const uint32_t d = dstv[k], ml = mlen[k];
+                        const uint32_t dmv = dm[k], d = dmv & 0xFFFFu, ml = dmv >> 16;
                         const unsigned long long sp = delta[2 * k + 2] + d, dp = outB + d;
                         for (uint32_t j = tid & 7u; j < ml; j += 8)
                             *reinterpret_cast<uint8_t *>(dp + j) = (uint8_t)ldg_u8(sp + j);
                     }
+                    i0 = i1;
                 }
             }
         }
         // publish (also for a bad block: later blocks must not wait forever)
+        __syncthreads();
+        TRACE_MARK(5);
         __threadfence();
         __syncthreads();
-        if (tid < 32) {
-            if (tid == 0) st_release_u32(done + blk, epoch);
-            __syncwarp();
-            advance_watermark(ctl, done, cv.n_blocks, epoch);
-        }
+        TRACE_MARK(6);
+        if (warp == 0) publish_block(ctl, done, cv.n_blocks, epoch, blk);
+        TRACE_MARK(7);
     }
     // last CTA out re-arms the ticket for the next launch
     if (tid == 0) {

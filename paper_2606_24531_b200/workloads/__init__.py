@@ -75,7 +75,7 @@ class Config:
 # >= 4 bytes, no scheduling promises); `scheduled` is the policy the large configs run with
 # (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks.
 POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
-POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64)
+POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1)
 
 CONFIGS = {
     "markov_1m": Config("markov_1m", "markov", 1 * MIB, SEED_BASE + 1, 4, POLICY_LITERAL,
