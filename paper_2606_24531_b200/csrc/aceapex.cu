@@ -288,7 +288,7 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         if (rc != ACEAPEX_OK) return rc;
         {
             LaunchScope ls(c, K_MATCH, st);
-            k_match<<<count, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
+            k_match<<<count + 1, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
                                                                     static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
                                                                     c->sc.done, c->epoch);
         }

@@ -284,6 +284,13 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, Sl
         SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
         const Record r = open_record(cv, blk);
         bool ok = r.ok;
+        if (s == LIT && ok && lane == 0) {
+            hdr->n_seq = r.n_seq; hdr->n_lit = r.n_lit; hdr->block_len = r.block_len;
+            hdr->n_extras = r.n_extras; hdr->off_nbytes = r.off_nbytes;
+            hdr->extras_off = r.extras_off; hdr->tags_off = r.tags_off;
+            const uint64_t ro = (uint64_t)(r.rec - cv.payload);
+            hdr->rec_lo = (uint32_t)ro; hdr->rec_hi = (uint32_t)(ro >> 32);
+        }
         if (ok) {
             // a stream longer than its slot area cannot occur once open() has found max_n_seq,
             // but the check keeps the store loop in bounds for any input

@@ -138,11 +138,16 @@ struct SlotLayout {
 };
 
 struct SlotHdr {
-    uint32_t bad[3];     // per stream: entropy decode failed
+    uint32_t bad[3];     // per stream: entropy decode failed (bad[LIT] also: record header invalid)
     uint32_t n_seq, n_lit, block_len;
     uint32_t parsed_ok;  // k_parse: tokens valid
-    uint32_t pad;
+    // record header fields, written by the entropy kernel's LIT unit so that the match kernel needs
+    // one 64-byte load instead of the rec_off -> record header chain
+    uint32_t n_extras, off_nbytes, extras_off, tags_off;
+    uint32_t rec_lo, rec_hi;   // record offset relative to the payload
+    uint32_t pad[3];
 };
+static_assert(sizeof(SlotHdr) == 64, "SlotHdr layout");
 
 __host__ inline SlotLayout make_slot_layout(uint32_t max_n_seq, uint32_t W)
 {

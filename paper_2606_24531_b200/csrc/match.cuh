@@ -133,44 +133,42 @@ __device__ inline void st_release_u32(uint32_t *p, uint32_t v)
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Publish block `blk` as complete and keep the watermark (number of leading complete blocks) moving.
-// Called by all 32 lanes of one warp after the block's bytes were fenced. Only the CTA that
-// completes the oldest outstanding block (watermark == blk) scans forward, 32 done flags per round
-// trip; everybody else sets its flag and leaves. The flag store and the watermark load, and on the
-// scanner's side the watermark store and the re-read of the next flag, are separated by
-// sequentially consistent fences (store-buffering pattern): whichever of the two CTAs comes second
-// sees the other's write, so the watermark never stalls below a completed block. Waiters acquire the
-// watermark; the scanner read the flags with acquire semantics and fenced before publishing it, so
-// a waiter also sees those blocks' bytes.
-__device__ inline void publish_block(Control *ctl, uint32_t *done, uint64_t n_blocks, uint32_t epoch, uint64_t blk)
+// Cross-block ordering. A finished block publishes its done flag (epoch of this call) with release
+// semantics; the flag store follows the CTA barrier that ends the block's writes, and a release is
+// cumulative over what the barrier ordered before it, so one thread publishes for the whole CTA.
+// The watermark (number of leading complete blocks) is advanced lazily by whoever needs it: a CTA
+// whose block copies from earlier blocks scans the done flags from the watermark on, 32 per round
+// trip with acquire loads, until everything below its highest source block is complete, and leaves
+// the new watermark behind for the next one (atomicMax after a fence, so that a later reader of the
+// watermark also sees those blocks' bytes). Block ids are handed out in increasing order, so every
+// block a CTA waits for belongs to a CTA that is running or finished: no deadlock.
+//
+// When the header promises a window R, a block knows before it has parsed anything that its sources
+// end below block blk - R + 1: one warp runs the scan up to there while the block's streams are still
+// in flight (blocking = false: it stops at the first incomplete block instead of spinning), and the
+// blocking call after the parse usually finds nothing left to do.
+__device__ inline unsigned long long wait_for_blocks(Control *ctl, const uint32_t *done, uint32_t epoch,
+                                                     unsigned long long w, unsigned long long below, bool blocking)
 {
     const uint32_t lane = lane_id();
-    unsigned long long w = 0;
-    if (lane == 0) {
-        st_release_u32(done + blk, epoch);
+    const unsigned long long w0 = w;
+    while (w < below) {
+        const unsigned long long idx = w + lane;
+        const bool f = idx >= below || ld_acquire_u32(done + idx) == epoch;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
+        if (m == 0xFFFFFFFFu) {
+            w = w + 32 < below ? w + 32 : below;
+        } else {
+            w += (uint32_t)__ffs(~m) - 1u;
+            if (!blocking) break;
+            __nanosleep(200);
+        }
+    }
+    if (w > w0 && lane == 0) {
         __threadfence();
-        w = ld_acquire_u64(&ctl->watermark);
+        atomicMax(&ctl->watermark, w);
     }
-    w = __shfl_sync(0xFFFFFFFFu, w, 0);
-    if (w != blk) return;
-    for (;;) {
-        for (;;) {
-            const unsigned long long idx = w + lane;
-            const bool f = idx < n_blocks && ld_acquire_u32(done + idx) == epoch;
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
-            const uint32_t c = m == 0xFFFFFFFFu ? 32u : (uint32_t)__ffs(~m) - 1u;
-            w += c;
-            if (c < 32) break;
-        }
-        uint32_t again = 0;
-        if (lane == 0) {
-            __threadfence();
-            atomicMax(&ctl->watermark, w);
-            __threadfence();
-            again = w < n_blocks && ld_acquire_u32(done + w) == epoch;
-        }
-        if (!__shfl_sync(0xFFFFFFFFu, again, 0)) return;
-    }
+    return w;
 }
 
 // ---- decode_all match kernel --------------------------------------------------------------------
@@ -247,11 +245,17 @@ __device__ inline Addr4 run_addresses(const uint2 *bm2, const uint16_t *rk, cons
     const uint32_t r1 = r0 + ((t >> 1) & 1u) + ((u >> 1) & 1u);
     const uint32_t r2 = r1 + ((t >> 2) & 1u) + ((u >> 2) & 1u);
     const uint32_t r3 = r2 + ((t >> 3) & 1u) + ((u >> 3) & 1u);
+    // Most groups lie in one run or straddle one boundary: the first and the last entry are always
+    // loaded, the middle ones only when they differ from both (the shared-memory pipe is the busy one).
+    const unsigned long long d0 = delta[r0], d3 = delta[r3];
+    unsigned long long d1 = r1 == r0 ? d0 : d3, d2 = r2 == r0 ? d0 : d3;
+    if (r1 != r0 && r1 != r3) d1 = delta[r1];
+    if (r2 != r0 && r2 != r3) d2 = delta[r2];
     Addr4 a;
-    a.a0 = delta[r0] + o;
-    a.a1 = delta[r1] + o + 1;
-    a.a2 = delta[r2] + o + 2;
-    a.a3 = delta[r3] + o + 3;
+    a.a0 = d0 + o;
+    a.a1 = d1 + o + 1;
+    a.a2 = d2 + o + 2;
+    a.a3 = d3 + o + 3;
     return a;
 }
 
@@ -276,6 +280,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     __shared__ uint32_t ws3[kMatchWarps][3];
     __shared__ uint32_t ws2[kMatchWarps][2];
     __shared__ uint32_t s_ticket, s_ntag, s_bad, s_below;
+    __shared__ unsigned long long s_wm;
     __shared__ uint32_t s_cnt[16], s_cur[16];
 
     const uint32_t ms = sl.ms;
@@ -299,19 +304,53 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     }
     if (tid < 16) s_cnt[tid] = 0;
     for (uint32_t i = tid; i < 256; i += kMatchThreads) reinterpret_cast<uint4 *>(bm2)[i] = make_uint4(0, 0, 0, 0);
-    unsigned long long wm_early = 0;                                   // thread 0: the watermark as of now (it only grows)
-    if (tid == 0) wm_early = ld_acquire_u64(&ctl->watermark);
     __syncthreads();
-    const uint32_t bi = s_ticket;
     TRACE_DECL;
+    if (s_ticket == 0) {
+        // Ticket 0 (a CTA that is certainly running) does not decode a block: its first warp keeps the
+        // watermark moving for everybody, 32 done flags per round trip, until this launch's blocks are done.
+        const unsigned long long end = first + count;
+        if (tid == 0) s_wm = ld_acquire_u64(&ctl->watermark);
+        __syncthreads();
+        unsigned long long w = s_wm;
+        while (w < end) {
+            const unsigned long long idx = w + tid;
+            const bool f = idx >= end || ld_acquire_u32(done + idx) == epoch;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, f);
+            if (lane == 0) ws2[warp][0] = m == 0xFFFFFFFFu ? 32u : (uint32_t)__ffs(~m) - 1u;
+            __syncthreads();
+            uint32_t lead = 0;
+#pragma unroll
+            for (uint32_t i = 0; i < kMatchWarps; i++) {
+                const uint32_t c = ws2[i][0];
+                if (lead == 32 * i) lead += c;                         // only while every earlier warp was complete
+            }
+            __syncthreads();
+            if (lead) {
+                w = w + lead < end ? w + lead : end;
+                if (tid == 0) { __threadfence(); atomicMax(&ctl->watermark, w); }
+            } else {
+                __nanosleep(300);
+            }
+        }
+    }
+    const uint32_t bi = s_ticket - 1;                                  // ticket 0 -> 0xFFFFFFFF: no block
     if (bi < count) {
         const uint64_t blk = first + bi;
         const uint64_t B0 = blk << kBlockLog2;
         const uint8_t *slot = slots + (size_t)bi * sl.stride;
-        const SlotHdr *hdr = reinterpret_cast<const SlotHdr *>(slot + sl.o_hdr);
-        const Record r = open_record(cv, blk);
-        bool ok = r.ok && !(hdr->bad[0] | hdr->bad[1] | hdr->bad[2]) && r.n_seq <= ms;
-        const uint32_t n = r.n_seq, blen = r.block_len;
+        // the record header fields as the entropy kernel's LIT unit left them in the slot header
+        struct { const uint8_t *rec; uint32_t n_seq, n_lit, block_len, n_extras, off_nbytes, extras_off, tags_off; bool ok; } r;
+        {
+            const uint4 *hp = reinterpret_cast<const uint4 *>(slot + sl.o_hdr);
+            const uint4 h0 = hp[0], h1 = hp[1], h2 = hp[2], h3 = hp[3];
+            r.ok = !(h0.x | h0.y | h0.z);                              // bad[LIT] covers an invalid record header
+            r.n_seq = h0.w; r.n_lit = h1.x; r.block_len = h1.y;
+            r.n_extras = h1.w; r.off_nbytes = h2.x; r.extras_off = h2.y; r.tags_off = h2.z;
+            r.rec = cv.payload + ((uint64_t)h2.w | (uint64_t)h3.x << 32);
+        }
+        bool ok = r.ok && r.n_seq <= ms;
+        const uint32_t n = ok ? r.n_seq : 0, blen = ok ? r.block_len : 0;
         TRACE_MARK(0);
         if (ok) {
             // ---- parse (FORMAT.md section 4). Warp w owns the sequences [w*cw, (w+1)*cw), lane-strided:
@@ -328,14 +367,19 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 for (uint32_t i = tid; i < no; i += kMatchThreads) cp_async16(s_off + 16 * i, go + 16 * i);
                 for (uint32_t i = tid; i < nt; i += kMatchThreads) cp_async16(s_tags + 16 * i, gt + 16 * i);
                 cp_async_commit();
+                if (tid == kMatchThreads - 1) s_wm = ld_acquire_u64(&ctl->watermark);   // it only grows; overlapped with the copies
                 cp_async_wait_all();
                 __syncthreads();
+                TRACE_MARK(8);
             }
             const uint16_t *len16 = s_len16;
             const uint8_t *off_s = s_off;
             const uint16_t *extras = reinterpret_cast<const uint16_t *>(r.rec + r.extras_off);
             const uint8_t *tagsec = s_tags;
             const bool has_esc = r.n_extras != 0;                      // CTA-uniform
+            // true (lit_len | match_len << 16) per sequence of a block with length escapes (rare): kept in the
+            // slot's o_src area, which only the isolated path uses otherwise
+            uint32_t *esc_val = reinterpret_cast<uint32_t *>(const_cast<uint8_t *>(slot) + sl.o_src);
             // A0 (only with escapes): escapes per warp -> extras base of each warp
             uint32_t esc_base = 0;
             if (has_esc) {
@@ -353,14 +397,16 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 ok = tot == r.n_extras;
                 __syncthreads();
             }
-            // A: sums per warp
+            // A: one packed warp scan per round. dm[k] receives the warp-relative exclusive prefix
+            //    (literals before k | bytes before k << 16); the warp totals go to shared memory.
             uint32_t sum_ll = 0, sum_all = 0, any_esc = 0;
             if (ok) {
-                uint32_t e_carry = esc_base;
+                uint32_t e_carry = esc_base, carry = 0;
                 for (uint32_t kb = wk0; kb < wk1; kb += 32) {
                     const uint32_t k = kb + lane;
+                    const bool act = k < wk1;
                     uint32_t ll = 0, ml = 0;
-                    if (k < wk1) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
+                    if (act) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
                     const uint32_t e_ll = ll == 255, e_ml = ml == 259;
                     any_esc |= e_ll | e_ml;
                     if (has_esc) {
@@ -369,7 +415,12 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                         if (e_ll) ll = extras[e++];
                         if (e_ml) ml = (uint32_t)extras[e] + 4;
                         e_carry += etot;
+                        if (act) esc_val[k] = ll | ml << 16;            // true lengths for pass B
                     }
+                    uint32_t ptot;
+                    const uint32_t pre = warp_excl_scan(ll | (ll + ml) << 16, lane, ptot);
+                    if (act) dm[k] = carry + pre;
+                    carry += ptot;
                     sum_ll += ll;
                     sum_all += ll + ml;
                 }
@@ -379,6 +430,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 if (lane == 0) { ws3[warp][0] = sum_ll; ws3[warp][1] = sum_all; ws3[warp][2] = any_esc; }
             }
             __syncthreads();
+            TRACE_MARK(9);
             uint32_t ll_base = 0, all_base = 0, ll_total = 0, all_total = 0;
             if (ok) {
                 uint32_t esc_seen = 0;
@@ -391,36 +443,26 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 ok = ll_total <= r.n_lit && all_total + (r.n_lit - ll_total) == blen && (has_esc || !esc_seen);
             }
             if (ok) {
-                // B: positions, run table, bitmaps, tag list. Every partial sum is <= 16384 now.
+                // B: elementwise. Every partial sum is <= block_len <= 16384 now, so st, d < 16384.
                 const unsigned long long lit_a = (unsigned long long)__cvta_generic_to_global(slot + sl.o_lit);
                 const unsigned long long out_a = (unsigned long long)__cvta_generic_to_global(out);
                 const uint32_t onb = r.off_nbytes;                     // 1..8
                 const uint64_t src_mask = ~0ull >> (64 - 8 * onb);
+                const uint32_t blk32 = (uint32_t)blk;                  // n_blocks < 2^32 (checked by open)
                 bool bad = false;
-                uint64_t mx = 0;                                       // max end of a source range that starts below B0
-                uint32_t e_carry = esc_base, lp_carry = ll_base, pos_carry = all_base;
+                uint32_t below = 0;                                    // 1 + highest earlier block read (upper bound)
+                const uint32_t base = ll_base | all_base << 16;
                 for (uint32_t kb = wk0; kb < wk1; kb += 32) {
                     const uint32_t k = kb + lane;
-                    const bool act = k < wk1;
-                    uint32_t ll = 0, ml = 0;
-                    if (act) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
-                    if (has_esc) {
-                        const uint32_t e_ll = ll == 255, e_ml = ml == 259;
-                        uint32_t etot;
-                        uint32_t e = e_carry + warp_excl_scan(e_ll + e_ml, lane, etot);
-                        if (e_ll) ll = extras[e++];
-                        if (e_ml) ml = (uint32_t)extras[e] + 4;
-                        e_carry += etot;
-                    }
-                    uint32_t ptot;
-                    const uint32_t pre = warp_excl_scan(ll | (ll + ml) << 16, lane, ptot);
-                    const uint32_t lp = lp_carry + (pre & 0xFFFFu);    // first literal of sequence k
-                    const uint32_t st = pos_carry + (pre >> 16);       // in-block offset where sequence k starts
-                    const uint32_t d = st + ll;                        // ... and where its match starts
-                    lp_carry += ptot & 0xFFFFu;
-                    pos_carry += ptot >> 16;
                     uint32_t tg = 0;
-                    if (act) {
+                    if (k < wk1) {
+                        uint32_t ll, ml;
+                        if (has_esc) { const uint32_t v = esc_val[k]; ll = v & 0xFFFFu; ml = v >> 16; }
+                        else { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
+                        const uint32_t pre = dm[k] + base;
+                        const uint32_t lp = pre & 0xFFFFu;             // first literal of sequence k
+                        const uint32_t st = pre >> 16;                 // in-block offset where sequence k starts
+                        const uint32_t d = st + ll;                    // ... and where its match starts
                         // src = the onb bytes at off_s[k * onb]: three aligned words, funnel-shifted and masked
                         const uint32_t p = k * onb, sh = (p & 3u) * 8;
                         const uint32_t *wp = reinterpret_cast<const uint32_t *>(off_s + (p & ~3u));
@@ -428,12 +470,14 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                         const uint32_t lo = __funnelshift_r(w0, w1, sh), hi = __funnelshift_r(w1, w2, sh);
                         const uint64_t src = (((uint64_t)hi << 32) | lo) & src_mask;
                         tg = (tagsec[k >> 1] >> ((k & 1) * 4)) & 15u;
-                        if (st < kB) atomicOr(&bm2[st >> 5].x, 1u << (st & 31));
-                        if (d < kB) atomicOr(&bm2[d >> 5].y, 1u << (d & 31));
+                        atomicOr(&bm2[st >> 5].x, 1u << (st & 31));
+                        atomicOr(&bm2[d >> 5].y, 1u << (d & 31));
                         *reinterpret_cast<ulonglong2 *>(&delta[2 * k + 1]) = make_ulonglong2(lit_a + lp - st, out_a + src - d);
                         dm[k] = d | ml << 16;
                         if (src + ml > B0 + d) bad = true;             // strictly before, non-overlapping
-                        if (src < B0 && src + ml > mx) mx = src + ml;
+                        // a source that starts in block sb < blk ends in block sb or sb + 1 (ml <= 16384)
+                        const uint64_t sb = src >> kBlockLog2;
+                        if (sb < blk) below = max(below, min((uint32_t)sb + 2u, blk32));
                     }
                     const uint32_t tm = __ballot_sync(0xFFFFFFFFu, tg != 0);
                     if (tm) {                                          // warp-aggregated append to the tag list
@@ -450,8 +494,6 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                     if (all_total < blen) atomicOr(&bm2[all_total >> 5].x, 1u << (all_total & 31));
                     delta[2 * n + 1] = lit_a + ll_total - all_total;
                 }
-                uint32_t below = 0;                                    // 1 + highest earlier block read
-                if (mx) below = (uint32_t)(((mx < B0 ? mx : B0) - 1) >> kBlockLog2) + 1;
                 below = __reduce_max_sync(0xFFFFFFFFu, below);
                 if (lane == 0 && below) atomicMax(&s_below, below);
                 if (__any_sync(0xFFFFFFFFu, bad) && lane == 0) s_bad = 1;
@@ -460,9 +502,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             TRACE_MARK(1);
             ok = ok && !s_bad;
             if (!ok && tid == 0) raise(ctl, kStTokens, blk);
-        } else if (tid == 0 && !r.ok) {
-            raise(ctl, kStRecord, blk);
-        }
+        }                                                              // (a bad record or stream was raised by k_entropy)
         if (ok) {
             // rk[w] = number of S and D bits in the words before w; tag list sorted by level
             {
@@ -476,7 +516,10 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 if (tid < 256) reinterpret_cast<uint32_t *>(rk)[tid] = r0 | (r0 + p0) << 16;
             }
             const uint32_t ntag = s_ntag;
-            if (ntag) {
+            const bool one_level = s_cnt[1] == ntag;                   // every tagged match has tag 1: no sorting
+            const uint16_t *lst = tlist;
+            if (!one_level) {
+                __syncthreads();                                       // everybody has read s_cnt[1]
                 if (tid == 0) {
                     uint32_t acc = 0;
                     for (int t = 0; t < 16; t++) { s_cur[t] = acc; acc += s_cnt[t]; s_cnt[t] = acc; }   // s_cnt[t] = end of level t
@@ -486,13 +529,12 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                     const uint32_t e = tlist[i];
                     slist[atomicAdd(&s_cur[e >> 12], 1u)] = (uint16_t)e;
                 }
+                lst = slist;
             }
             // wait until every earlier block this block copies from is complete
             const uint64_t below = s_below;
             TRACE_MARK(2);
-            if (tid == 0) {
-                while (wm_early < below) { __nanosleep(100); wm_early = ld_acquire_u64(&ctl->watermark); }
-            }
+            if (warp == 0 && s_wm < below) wait_for_blocks(ctl, done, epoch, s_wm, below, true);
             __syncthreads();
             TRACE_MARK(3);
             // ---- pass 0: every output byte from delta[r(o)] + o; 16 byte loads in flight per thread
@@ -523,17 +565,16 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
                 *reinterpret_cast<uint8_t *>(outB + o) = (uint8_t)ldg_u8(delta[r0] + o);
             }
-            __syncthreads();
             TRACE_MARK(4);
             // ---- matches whose source reaches into this block, level by level, 8 lanes per match
             if (ntag) {
                 uint32_t i0 = 0;
                 for (uint32_t level = 1; level < 16 && i0 < ntag; level++) {
-                    const uint32_t i1 = s_cnt[level];
+                    const uint32_t i1 = one_level ? ntag : s_cnt[level];
                     if (i0 == i1) continue;                            // CTA-uniform
                     __syncthreads();                                   // the previous level (or pass 0) is in place
                     for (uint32_t i = i0 + (tid >> 3); i < i1; i += kMatchThreads / 8) {
-                        const uint32_t k = slist[i] & 0xFFFu;
+                        const uint32_t k = lst[i] & 0xFFFu;
                         const uint32_t dmv = dm[k], d = dmv & 0xFFFFu, ml = dmv >> 16;
                         const unsigned long long sp = delta[2 * k + 2] + d, dp = outB + d;
                         for (uint32_t j = tid & 7u; j < ml; j += 8)
@@ -546,10 +587,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         // publish (also for a bad block: later blocks must not wait forever)
         __syncthreads();
         TRACE_MARK(5);
-        __threadfence();
-        __syncthreads();
-        TRACE_MARK(6);
-        if (warp == 0) publish_block(ctl, done, cv.n_blocks, epoch, blk);
+        if (tid == 0) st_release_u32(done + blk, epoch);
         TRACE_MARK(7);
     }
     // last CTA out re-arms the ticket for the next launch
