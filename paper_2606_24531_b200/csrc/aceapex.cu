@@ -32,6 +32,7 @@ struct aceapex_ctx {
     uint32_t epoch = 0, tag = 0;
     uint64_t launches = 0;
     int sm_count = 0;
+    int match_ctas_per_sm = 0;
     int device = 0;
     bool prof = false;
     std::vector<ProfRec> prof_recs;
@@ -92,6 +93,20 @@ inline uint32_t block_len_host(const aceapex_ctx *c, uint64_t b)
 
 inline size_t entropy_smem() { return kEntropySmem; }
 inline size_t match_smem(const aceapex_ctx *c) { return match_smem_bytes(c->sl.ms, c->cv.W); }
+
+// Persistent match kernel: as many CTAs as fit on the device at once (plus nothing: the helper that
+// keeps the watermark is one of them), but never more than blocks + 1.
+uint32_t match_grid(aceapex_ctx *c, uint32_t count)
+{
+    if (c->match_ctas_per_sm == 0) {
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_match, (int)kMatchThreads, match_smem(c)) != cudaSuccess || nb < 1) nb = 1;
+        c->match_ctas_per_sm = nb;
+    }
+    const uint64_t cap = (uint64_t)c->match_ctas_per_sm * (uint64_t)c->sm_count;
+    const uint64_t want = (uint64_t)count + 1;
+    return (uint32_t)(want < cap ? want : cap);
+}
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
                    uint32_t count, cudaStream_t st)
@@ -288,7 +303,7 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         if (rc != ACEAPEX_OK) return rc;
         {
             LaunchScope ls(c, K_MATCH, st);
-            k_match<<<count + 1, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
+            k_match<<<match_grid(c, count), kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
                                                                     static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
                                                                     c->sc.done, c->epoch);
         }

@@ -296,6 +296,9 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t lt = (1u << lane) - 1u;
+  // Persistent CTAs: each takes block after block from the ticket counter until none is left.
+  for (;;) {
+    __syncthreads();                                                   // the previous block's shared state is dead
     if (tid == 0) {
         s_ticket = atomicAdd(&ctl->ticket, 1u);
         s_below = 0;
@@ -305,6 +308,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     if (tid < 16) s_cnt[tid] = 0;
     for (uint32_t i = tid; i < 256; i += kMatchThreads) reinterpret_cast<uint4 *>(bm2)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
+    if (s_ticket > count) break;                                       // tickets 1 .. count are blocks
     TRACE_DECL;
     if (s_ticket == 0) {
         // Ticket 0 (a CTA that is certainly running) does not decode a block: its first warp keeps the
@@ -573,12 +577,46 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                     const uint32_t i1 = one_level ? ntag : s_cnt[level];
                     if (i0 == i1) continue;                            // CTA-uniform
                     __syncthreads();                                   // the previous level (or pass 0) is in place
-                    for (uint32_t i = i0 + (tid >> 3); i < i1; i += kMatchThreads / 8) {
-                        const uint32_t k = lst[i] & 0xFFFu;
-                        const uint32_t dmv = dm[k], d = dmv & 0xFFFFu, ml = dmv >> 16;
-                        const unsigned long long sp = delta[2 * k + 2] + d, dp = outB + d;
-                        for (uint32_t j = tid & 7u; j < ml; j += 8)
-                            *reinterpret_cast<uint8_t *>(dp + j) = (uint8_t)ldg_u8(sp + j);
+                    // 8 lanes per match, 4 matches per step: the first 16 bytes of each (2 per lane) are loaded
+                    // before any is stored, so a step costs one round trip instead of four
+                    const uint32_t l8 = tid & 7u, G = kMatchThreads / 8;
+                    for (uint32_t ib = i0 + (tid >> 3); ib < i1; ib += 4 * G) {
+                        unsigned long long sp[4], dp[4];
+                        uint32_t ml[4], v0[4], v1[4];
+#pragma unroll
+                        for (int u = 0; u < 4; u++) {
+                            const uint32_t i = ib + u * G;
+                            ml[u] = 0; sp[u] = dp[u] = 0;
+                            if (i < i1) {
+                                const uint32_t k = lst[i] & 0xFFFu;
+                                const uint32_t dmv = dm[k], d = dmv & 0xFFFFu;
+                                ml[u] = dmv >> 16;
+                                sp[u] = delta[2 * k + 2] + d; dp[u] = outB + d;
+                            }
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; u++) {
+                            v0[u] = l8 < ml[u] ? ldg_u8(sp[u] + l8) : 0;
+                            v1[u] = l8 + 8 < ml[u] ? ldg_u8(sp[u] + l8 + 8) : 0;
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; u++) {
+                            if (l8 < ml[u]) *reinterpret_cast<uint8_t *>(dp[u] + l8) = (uint8_t)v0[u];
+                            if (l8 + 8 < ml[u]) *reinterpret_cast<uint8_t *>(dp[u] + l8 + 8) = (uint8_t)v1[u];
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; u++) {                  // the rest of a long match, 4 loads in flight
+                            for (uint32_t j = 16 + l8; j < ml[u]; j += 32) {
+                                const uint32_t a = ldg_u8(sp[u] + j);
+                                const uint32_t b = j + 8 < ml[u] ? ldg_u8(sp[u] + j + 8) : 0;
+                                const uint32_t c = j + 16 < ml[u] ? ldg_u8(sp[u] + j + 16) : 0;
+                                const uint32_t e = j + 24 < ml[u] ? ldg_u8(sp[u] + j + 24) : 0;
+                                *reinterpret_cast<uint8_t *>(dp[u] + j) = (uint8_t)a;
+                                if (j + 8 < ml[u]) *reinterpret_cast<uint8_t *>(dp[u] + j + 8) = (uint8_t)b;
+                                if (j + 16 < ml[u]) *reinterpret_cast<uint8_t *>(dp[u] + j + 16) = (uint8_t)c;
+                                if (j + 24 < ml[u]) *reinterpret_cast<uint8_t *>(dp[u] + j + 24) = (uint8_t)e;
+                            }
+                        }
                     }
                     i0 = i1;
                 }
@@ -590,6 +628,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         if (tid == 0) st_release_u32(done + blk, epoch);
         TRACE_MARK(7);
     }
+  }
     // last CTA out re-arms the ticket for the next launch
     if (tid == 0) {
         __threadfence();
