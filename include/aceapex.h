@@ -21,10 +21,9 @@
  *     position, ...) never cause an out-of-bounds access: the offending block is left
  *     unwritten, a sticky status word is set in device memory and aceapex_device_status()
  *     returns ACEAPEX_E_CORRUPT.
- *   - decode_all is asynchronous on `cuda_stream`. decode_blocks / seek are stream-ordered; they
- *     synchronise the stream internally once per copy hop (they read one counter back) unless
- *     the container header promises a copy depth D (FORMAT.md section 1), in which case they
- *     enqueue D+1 hops and return without synchronising.
+ *   - Every decode call is asynchronous on `cuda_stream`: decode_all enqueues two kernels per
+ *     batch of n_slots blocks, decode_blocks / seek one fused kernel per group of n_targets
+ *     blocks (the copy-hop loop runs on the device and ends there; no host read-back).
  *   - There is no CPU fallback: without a CUDA device every call except aceapex_strerror and
  *     aceapex_version fails with ACEAPEX_E_CUDA.
  */
@@ -90,7 +89,8 @@ int aceapex_info_get(const aceapex_ctx *ctx, aceapex_info *out);
 /* Scratch the caller must provide (DEVICE, 256-byte aligned) for the given batch limits.
  *   n_slots    decoded-token slots: blocks whose token streams are resident at once. decode_all
  *              works through the container in batches of n_slots blocks; decode_blocks / seek
- *              use one slot per distinct block touched in a hop. >= 1.
+ *              use one slot per distinct block touched by a group of targets (with fewer slots
+ *              they still decode correctly, in several rounds). >= 1.
  *   n_targets  target blocks whose per-byte chase state is resident at once in decode_blocks
  *              (the id list is processed in groups of n_targets); 0 if only decode_all is used.
  * Returns 0 on a NULL context. */

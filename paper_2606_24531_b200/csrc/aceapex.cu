@@ -12,11 +12,8 @@
 
 using namespace aceapex;
 
-enum KernelId { K_SCAN = 0, K_ENTROPY, K_MATCH, K_EXPORT, K_SEEK_INIT, K_SEEK_COLLECT, K_PARSE, K_SEEK_RESOLVE,
-                K_SEEK_CHECK, K_COUNT };
-static const char *const kKernelNames[K_COUNT] = { "k_scan_records", "k_entropy", "k_match", "k_export_streams",
-                                                   "k_seek_init", "k_seek_collect", "k_parse", "k_seek_resolve",
-                                                   "k_seek_check" };
+enum KernelId { K_SCAN = 0, K_ENTROPY, K_MATCH, K_EXPORT, K_SEEK_FUSED, K_COUNT };
+static const char *const kKernelNames[K_COUNT] = { "k_scan_records", "k_entropy", "k_match", "k_export_streams", "k_seek_fused" };
 static_assert(K_COUNT <= ACEAPEX_N_KERNELS, "kernel id table");
 
 struct ProfRec { int id; cudaEvent_t e0, e1; };
@@ -28,11 +25,11 @@ struct aceapex_ctx {
     Scratch sc{};
     bool have_scratch = false;
     Control *open_ctl = nullptr;          // tiny internal allocation used by the open-time scan
-    unsigned long long *h_pending = nullptr;  // pinned, hop-loop read-back
     uint32_t epoch = 0, tag = 0;
     uint64_t launches = 0;
     int sm_count = 0;
     int match_ctas_per_sm = 0;
+    int seek_ctas_per_sm = 0;
     int device = 0;
     bool prof = false;
     std::vector<ProfRec> prof_recs;
@@ -191,7 +188,6 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
     c->cv.payload_bytes = edge[1];
 
     if (rc == ACEAPEX_OK && cudaMalloc(&c->open_ctl, sizeof(Control)) != cudaSuccess) rc = ACEAPEX_E_CUDA;
-    if (rc == ACEAPEX_OK && cudaMallocHost(&c->h_pending, 64) != cudaSuccess) rc = ACEAPEX_E_CUDA;
     if (rc == ACEAPEX_OK) {
         Control init;
         memset(&init, 0, sizeof init);
@@ -210,7 +206,8 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
     if (rc == ACEAPEX_OK && cudaMemcpy(&res, c->open_ctl, sizeof res, cudaMemcpyDeviceToHost) != cudaSuccess) rc = ACEAPEX_E_CUDA;
     if (rc == ACEAPEX_OK && res.status) rc = ACEAPEX_E_CORRUPT;
     if (rc == ACEAPEX_OK) {
-        if (cudaFuncSetAttribute(k_entropy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)entropy_smem()) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_entropy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)entropy_smem()) != cudaSuccess ||
+            cudaFuncSetAttribute(k_seek_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)entropy_smem()) != cudaSuccess)
             rc = ACEAPEX_E_CUDA;
     }
     if (rc != ACEAPEX_OK) { aceapex_close(c); return rc; }
@@ -237,7 +234,6 @@ void aceapex_close(aceapex_ctx *c)
 {
     if (!c) return;
     if (c->open_ctl) cudaFree(c->open_ctl);
-    if (c->h_pending) cudaFreeHost(c->h_pending);
     for (ProfRec &r : c->prof_recs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     delete c;
@@ -347,62 +343,44 @@ int aceapex_decode_blocks(aceapex_ctx *c, const uint64_t *h_ids, size_t n_ids, v
     }
     if (out_capacity < need) return ACEAPEX_E_CAPACITY;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    Control *ctl = c->sc.ctl;
     const uint32_t S = (uint32_t)(c->sc.n_slots > 0xFFFFFFFFull / 4 ? 0xFFFFFFFFull / 4 : c->sc.n_slots);
+    if (c->seek_ctas_per_sm == 0) {
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_seek_fused, 32 * (int)kEntropyWarps, entropy_smem()) != cudaSuccess || nb < 1)
+            return ACEAPEX_E_CUDA;
+        c->seek_ctas_per_sm = nb;
+    }
+    const uint32_t kMaxHops = 1u << 16;
 
     for (size_t base = 0; base < n_ids; base += c->sc.n_targets) {
         const uint32_t nt = (uint32_t)(n_ids - base < c->sc.n_targets ? n_ids - base : c->sc.n_targets);
-        const uint64_t n_bytes = (uint64_t)nt * kB;
-        if (cudaMemcpyAsync(c->sc.ids, h_ids + base, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess)
-            return ACEAPEX_E_CUDA;
-        {
-            LaunchScope ls(c, K_SEEK_INIT, st);
-            k_seek_init<<<(uint32_t)((n_bytes + 255) / 256), 256, 0, st>>>(c->cv, c->sc.ids, nt, c->sc.pend);
+        if (c->tag > 0xFFFFFFFFu - 2 * kMaxHops) {                     // hop tags would wrap: start over
+            if (cudaMemsetAsync(c->sc.mark, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+            c->tag = 0;
         }
-        // With a depth promise D and a slot for every block a hop can touch, D+1 hops always
-        // suffice (hop 0 resolves the target's own literals): enqueue them without reading back.
-        const uint64_t touch = n_bytes < c->cv.n_blocks ? n_bytes : c->cv.n_blocks;
-        const bool fixed = c->cv.D > 0 && (uint64_t)S >= touch;
-        const uint32_t chunks = (uint32_t)((n_bytes + kChunk - 1) / kChunk);
-        const uint32_t cgrid = (chunks + 127) / 128;
-        for (uint32_t hop = 0;; hop++) {
-            if (++c->tag == 0) {
-                if (cudaMemsetAsync(c->sc.mark, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-                c->tag = 1;
-            }
-            if (cudaMemsetAsync(&ctl->n_list, 0, 4, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-            if (cudaMemsetAsync(&ctl->pending, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-            {
-                LaunchScope ls(c, K_SEEK_COLLECT, st);
-                k_seek_collect<<<cgrid, 128, 0, st>>>(c->sc.pend, n_bytes, c->sc.mark, c->sc.slot_of, c->sc.list, ctl,
-                                                      c->tag, S);
-            }
-            int rc = launch_entropy(c, c->sc.list, &ctl->n_list, S, 0, 0, st);
-            if (rc != ACEAPEX_OK) return rc;
-            uint32_t pgrid = S < (uint32_t)c->sm_count * 8 ? S : (uint32_t)c->sm_count * 8;
-            {
-                LaunchScope ls(c, K_PARSE, st);
-                k_parse<<<pgrid, kMatchThreads, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.list, &ctl->n_list, S, ctl);
-            }
-            {
-                LaunchScope ls(c, K_SEEK_RESOLVE, st);
-                k_seek_resolve<<<cgrid, 128, 0, st>>>(c->cv, c->sl, c->sc.slots, c->sc.pend, nt, c->sc.ids, c->sc.mark,
-                                                      c->sc.slot_of, ctl, c->tag, S, static_cast<uint8_t *>(d_out),
-                                                      (uint64_t)base, absolute ? 1u : 0u);
-            }
-            if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
-            if (fixed) {
-                if (hop >= c->cv.D) {
-                    LaunchScope ls(c, K_SEEK_CHECK, st);
-                    k_seek_check<<<1, 1, 0, st>>>(ctl);
-                    break;
-                }
-            } else {
-                if (cudaMemcpyAsync(c->h_pending, &ctl->pending, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-                    return ACEAPEX_E_CUDA;
-                if (cudaStreamSynchronize(st) != cudaSuccess) return ACEAPEX_E_CUDA;
-                if (*c->h_pending == 0) break;
-            }
+        SeekArgs a;
+        a.pend = c->sc.pend; a.mark = c->sc.mark; a.slot_of = c->sc.slot_of; a.list = c->sc.list;
+        a.slots = c->sc.slots; a.out = static_cast<uint8_t *>(d_out);
+        a.out_base = (uint64_t)base; a.nt = nt; a.absolute = absolute ? 1u : 0u; a.max_slots = S;
+        a.tag0 = c->tag + 1; a.max_hops = kMaxHops;
+        c->tag += kMaxHops;
+        if (nt == 1) {
+            a.ids = nullptr; a.one_id = h_ids[base];                   // a single seek needs no copy at all
+        } else {
+            if (cudaMemcpyAsync(c->sc.ids, h_ids + base, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess)
+                return ACEAPEX_E_CUDA;
+            a.ids = c->sc.ids; a.one_id = 0;
+        }
+        // all CTAs must be co-resident (grid barrier): one CTA per SM for a few targets (cheaper
+        // barriers), the full occupancy for batches
+        uint32_t grid = (uint32_t)c->sm_count * (nt <= 4 ? 1u : (uint32_t)c->seek_ctas_per_sm);
+        Control *ctl = c->sc.ctl;
+        void *params[] = { &c->cv, &c->sl, &a, &ctl };
+        {
+            LaunchScope ls(c, K_SEEK_FUSED, st);
+            if (cudaLaunchCooperativeKernel((const void *)k_seek_fused, dim3(grid), dim3(32 * kEntropyWarps), params, entropy_smem(), st) !=
+                cudaSuccess)
+                return ACEAPEX_E_CUDA;
         }
     }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;

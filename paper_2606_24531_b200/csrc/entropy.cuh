@@ -246,6 +246,46 @@ __device__ inline bool decode_stream(uint32_t x /* this lane's initial state */,
     return __all_sync(0xFFFFFFFFu, x == kRansL) && wpos2 == wbytes;
 }
 
+// One (block, stream) unit, by one warp: stream s of block blk into slot bi. Output: the slot's stream
+// area and bad flag; with write_hdr also the record header fields in the slot header.
+__device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, uint8_t *slots, uint64_t blk, uint32_t bi,
+                                   int s, bool write_hdr, const WarpSmem &ws, uint32_t lane, Control *ctl)
+{
+    uint8_t *slot = slots + (size_t)bi * sl.stride;
+    SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
+    const Record r = open_record(cv, blk);
+    bool ok = r.ok;
+    if (write_hdr && ok && lane == 0) {
+        hdr->n_seq = r.n_seq; hdr->n_lit = r.n_lit; hdr->block_len = r.block_len;
+        hdr->n_extras = r.n_extras; hdr->off_nbytes = r.off_nbytes;
+        hdr->extras_off = r.extras_off; hdr->tags_off = r.tags_off;
+        const uint64_t ro = (uint64_t)(r.rec - cv.payload);
+        hdr->rec_lo = (uint32_t)ro; hdr->rec_hi = (uint32_t)(ro >> 32);
+    }
+    if (ok) {
+        // a stream longer than its slot area cannot occur once open() has found max_n_seq,
+        // but the check keeps the store loop in bounds for any input
+        const uint32_t cap = s == LIT ? kB : (s == LEN ? 2 * sl.ms : cv.W * sl.ms);
+        const uint32_t ns = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
+        if (ns > cap) ok = false;
+    }
+    if (ok) {
+        uint8_t *out = slot + (s == LIT ? sl.o_lit : (s == LEN ? sl.o_len : sl.o_off));
+        const uint32_t n = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
+        const uint32_t nw = s == LIT ? r.n_words[LIT] : (s == LEN ? r.n_words[LEN] : r.n_words[OFF]);
+        const uint32_t to = s == LIT ? r.tbl_off[LIT] : (s == LEN ? r.tbl_off[LEN] : r.tbl_off[OFF]);
+        const uint32_t tb = s == LIT ? r.tbl_bytes[LIT] : (s == LEN ? r.tbl_bytes[LEN] : r.tbl_bytes[OFF]);
+        const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
+        const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
+        ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
+        if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
+    } else if (lane == 0) {
+        raise(ctl, kStRecord, blk);
+    }
+    if (lane == 0) hdr->bad[s] = ok ? 0u : 1u;
+    __syncwarp();
+}
+
 // Kernel: every warp takes (block, stream) units from a counter until none is left.
 //   list != nullptr: the blocks are list[0 .. min(*n_list, max_slots)) (isolated path);
 //   else:            the blocks are first .. first+count-1.
@@ -279,40 +319,7 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, Sl
         // longest first: all LIT streams, then OFF, then LEN (balances the tail of the launch)
         const uint32_t so = u / nb, bi = u - so * nb;
         const int s = so == 0 ? LIT : (so == 1 ? OFF : LEN);
-        const uint64_t blk = list ? list[bi] : first + bi;
-        uint8_t *slot = slots + (size_t)bi * sl.stride;
-        SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
-        const Record r = open_record(cv, blk);
-        bool ok = r.ok;
-        if (s == LIT && ok && lane == 0) {
-            hdr->n_seq = r.n_seq; hdr->n_lit = r.n_lit; hdr->block_len = r.block_len;
-            hdr->n_extras = r.n_extras; hdr->off_nbytes = r.off_nbytes;
-            hdr->extras_off = r.extras_off; hdr->tags_off = r.tags_off;
-            const uint64_t ro = (uint64_t)(r.rec - cv.payload);
-            hdr->rec_lo = (uint32_t)ro; hdr->rec_hi = (uint32_t)(ro >> 32);
-        }
-        if (ok) {
-            // a stream longer than its slot area cannot occur once open() has found max_n_seq,
-            // but the check keeps the store loop in bounds for any input
-            const uint32_t cap = s == LIT ? kB : (s == LEN ? 2 * sl.ms : cv.W * sl.ms);
-            const uint32_t ns = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
-            if (ns > cap) ok = false;
-        }
-        if (ok) {
-            uint8_t *out = slot + (s == LIT ? sl.o_lit : (s == LEN ? sl.o_len : sl.o_off));
-            const uint32_t n = s == LIT ? r.n_sym[LIT] : (s == LEN ? r.n_sym[LEN] : r.n_sym[OFF]);
-            const uint32_t nw = s == LIT ? r.n_words[LIT] : (s == LEN ? r.n_words[LEN] : r.n_words[OFF]);
-            const uint32_t to = s == LIT ? r.tbl_off[LIT] : (s == LEN ? r.tbl_off[LEN] : r.tbl_off[OFF]);
-            const uint32_t tb = s == LIT ? r.tbl_bytes[LIT] : (s == LEN ? r.tbl_bytes[LEN] : r.tbl_bytes[OFF]);
-            const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
-            const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
-            ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
-            if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
-        } else if (lane == 0) {
-            raise(ctl, kStRecord, blk);
-        }
-        if (lane == 0) hdr->bad[s] = ok ? 0u : 1u;
-        __syncwarp();
+        decode_unit(cv, sl, slots, list ? list[bi] : first + bi, bi, s, s == LIT, ws, lane, ctl);
     }
     // last warp out re-arms the counters for the next launch
     if (lane == 0) {

@@ -117,9 +117,15 @@ struct Control {
     uint32_t status;                // sticky kSt* bits
     uint32_t ticket, ticket_exit;   // decode_all match kernel: ordered block hand-out
     uint32_t unit, unit_exit;       // entropy kernel: (block, stream) unit hand-out
-    uint32_t n_list;                // isolated decode: distinct blocks claimed in this hop
+    uint32_t n_list;                // (unused since the fused isolated kernel; kept for layout)
     uint32_t max_n_seq;             // open-time scan result
-    uint32_t pad[19];
+    // fused isolated decode (seek.cuh): grid barrier and per-hop counters, double-buffered by hop parity
+    uint32_t bar_count, bar_gen;
+    uint32_t round_n_list[2];       // distinct blocks claimed so far in the round (by round parity)
+    uint32_t hop_unit[2];           // (unused)
+    uint32_t pad0;
+    unsigned long long hop_pending[2];   // bytes still chasing after the hop (by hop parity)
+    uint32_t pad[8];
 };
 static_assert(sizeof(Control) == 128, "Control layout");
 
@@ -140,12 +146,13 @@ struct SlotLayout {
 struct SlotHdr {
     uint32_t bad[3];     // per stream: entropy decode failed (bad[LIT] also: record header invalid)
     uint32_t n_seq, n_lit, block_len;
-    uint32_t parsed_ok;  // k_parse: tokens valid
+    uint32_t parsed_ok;  // isolated decode: tokens parsed and valid
     // record header fields, written by the entropy kernel's LIT unit so that the match kernel needs
     // one 64-byte load instead of the rec_off -> record header chain
     uint32_t n_extras, off_nbytes, extras_off, tags_off;
     uint32_t rec_lo, rec_hi;   // record offset relative to the payload
-    uint32_t pad[3];
+    uint32_t need_lit;         // isolated decode: some chased byte ends on a literal of this block
+    uint32_t pad[2];
 };
 static_assert(sizeof(SlotHdr) == 64, "SlotHdr layout");
 
@@ -172,12 +179,12 @@ __host__ inline SlotLayout make_slot_layout(uint32_t max_n_seq, uint32_t W)
 struct Scratch {
     Control *ctl;
     uint32_t *done;      // [n_blocks] epoch of the decode_all call that completed the block
-    uint32_t *mark;      // [n_blocks] hop tag that claimed the block
-    uint32_t *slot_of;   // [n_blocks] slot index assigned in that hop
-    uint64_t *list;      // [n_slots]  block id held by each slot in this hop
+    uint32_t *mark;      // [n_blocks] tag of the isolated-decode round that claimed the block
+    uint32_t *slot_of;   // [n_blocks] slot index assigned in that round
+    uint64_t *list;      // [n_slots]  block id held by each slot in this round
     uint64_t *ids;       // [n_targets] target block ids of the current group
     uint8_t *slots;      // n_slots * stride
-    uint64_t *pend;      // [n_targets][16384] absolute position still to be chased, or kDone
+    uint64_t *pend;      // [n_targets][16384] absolute position still to be chased, literal request, or kDone
     uint64_t n_slots, n_targets;
 };
 

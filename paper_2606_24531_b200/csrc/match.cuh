@@ -9,111 +9,6 @@ namespace aceapex {
 constexpr uint32_t kMatchThreads = 256;
 constexpr uint32_t kMatchWarps = kMatchThreads / 32;
 
-// Token arrays of one block (shared memory in decode_all, the slot in the isolated path).
-struct Tokens {
-    uint16_t *start;   // [n_seq+1] in-block output offset where sequence k's literal run starts;
-                       //           entry n_seq = start of the trailing literals
-    uint16_t *dst;     // [n_seq]   in-block output offset of match k
-    uint16_t *litpos;  // [n_seq+1] index into LIT of sequence k's first literal
-    uint64_t *src;     // [n_seq]   absolute source position of match k
-    uint32_t *bm;      // optional [512]: bit o set iff some sequence (or the trailing run) starts at offset o
-};
-
-// Exclusive prefix sum of one value per thread over the CTA (kMatchThreads threads).
-__device__ inline uint32_t block_excl_scan(uint32_t v, uint32_t *warp_sums /* [kMatchWarps+1] smem */,
-                                           uint32_t &total)
-{
-    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-    uint32_t wtotal;
-    const uint32_t in_warp = warp_excl_scan(v, lane, wtotal);
-    __syncthreads();                       // warp_sums may still be read from a previous scan
-    if (lane == 0) warp_sums[warp] = wtotal;
-    __syncthreads();
-    uint32_t base = 0, tot = 0;
-#pragma unroll
-    for (uint32_t w = 0; w < kMatchWarps; w++) {
-        const uint32_t t = warp_sums[w];
-        if (w < warp) base += t;
-        tot += t;
-    }
-    total = tot;
-    return base + in_warp;
-}
-
-// Parse the decoded LEN / OFF streams of a block into token arrays (FORMAT.md section 4).
-// All kMatchThreads threads of the CTA call this. Returns true (CTA-uniform) iff every validity
-// rule holds: escapes consumed == n_extras, sum lit_len <= n_lit, sums == block_len, and for every
-// match src + match_len <= dst (absolute) — after which every copy below is in bounds.
-__device__ inline bool parse_tokens(const Record &r, uint64_t blk, const uint8_t *len_s, const uint8_t *off_s,
-                                    const Tokens &t, uint32_t *warp_sums, uint64_t *max_src_blk_below)
-{
-    const uint32_t n = r.n_seq;
-    const uint32_t per = (n + kMatchThreads - 1) / kMatchThreads;
-    const uint32_t k0 = min(n, threadIdx.x * per), k1 = min(n, k0 + per);
-    const uint16_t *extras = reinterpret_cast<const uint16_t *>(r.rec + r.extras_off);
-    const uint64_t B0 = blk << kBlockLog2;
-
-    uint32_t esc = 0;
-    for (uint32_t k = k0; k < k1; k++) esc += (len_s[2 * k] == 255) + (len_s[2 * k + 1] == 255);
-    uint32_t esc_total;
-    const uint32_t esc_base = block_excl_scan(esc, warp_sums, esc_total);
-    if (esc_total != r.n_extras) return false;               // CTA-uniform
-
-    uint32_t sum_ll = 0, sum_all = 0;
-    {
-        uint32_t e = esc_base;
-        for (uint32_t k = k0; k < k1; k++) {
-            uint32_t ll = len_s[2 * k], ml = len_s[2 * k + 1];
-            if (ll == 255) ll = extras[e++];
-            if (ml == 255) ml = extras[e++];
-            sum_ll += ll;
-            sum_all += ll + ml + 4;
-        }
-    }
-    uint32_t ll_total, all_total;
-    const uint32_t ll_base = block_excl_scan(sum_ll, warp_sums, ll_total);
-    const uint32_t all_base = block_excl_scan(sum_all, warp_sums, all_total);
-    if (ll_total > r.n_lit) return false;
-    if (all_total + (r.n_lit - ll_total) != r.block_len) return false;
-
-    bool bad = false;
-    uint64_t below = 0;                                      // 1 + highest earlier block read
-    {
-        uint32_t e = esc_base, lp = ll_base, pos = all_base;
-        for (uint32_t k = k0; k < k1; k++) {
-            uint32_t ll = len_s[2 * k], ml = len_s[2 * k + 1];
-            if (ll == 255) ll = extras[e++];
-            if (ml == 255) ml = extras[e++];
-            ml += 4;
-            uint64_t src = 0;
-            for (uint32_t j = 0; j < r.off_nbytes; j++) src |= (uint64_t)off_s[k * r.off_nbytes + j] << (8 * j);
-            t.start[k] = (uint16_t)pos;
-            t.litpos[k] = (uint16_t)lp;
-            if (t.bm && pos < kB) atomicOr(&t.bm[pos >> 5], 1u << (pos & 31));
-            pos += ll; lp += ll;
-            t.dst[k] = (uint16_t)pos;
-            t.src[k] = src;
-            if (src + ml > B0 + pos) bad = true;             // strictly before, non-overlapping
-            if (src < B0) {
-                const uint64_t last = (src + ml < B0 ? src + ml : B0) - 1;
-                const uint64_t need = (last >> kBlockLog2) + 1;
-                if (need > below) below = need;
-            }
-            pos += ml;
-        }
-    }
-    if (threadIdx.x == kMatchThreads - 1) {
-        t.start[n] = (uint16_t)all_total;
-        t.litpos[n] = (uint16_t)ll_total;
-        if (t.bm && all_total < kB) atomicOr(&t.bm[all_total >> 5], 1u << (all_total & 31));
-    }
-    if (max_src_blk_below) {
-        // CTA-wide max via shared atomics; caller zeroed *max_src_blk_below before the call
-        if (below) atomicMax(reinterpret_cast<unsigned long long *>(max_src_blk_below), (unsigned long long)below);
-    }
-    return !__syncthreads_or(bad);
-}
-
 // ---- cross-block ordering ---------------------------------------------------------------------
 
 __device__ inline uint32_t ld_acquire_u32(const uint32_t *p)
@@ -637,40 +532,6 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             ctl->ticket_exit = 0;
             __threadfence();
         }
-    }
-}
-
-// Isolated path: parse the tokens of every listed block into its slot (global memory).
-__global__ void __launch_bounds__(kMatchThreads) k_parse(Container cv, SlotLayout sl, uint8_t *slots,
-                                                          const uint64_t *list, const uint32_t *n_list,
-                                                          uint32_t max_slots, Control *ctl)
-{
-    __shared__ uint32_t warp_sums[kMatchWarps + 1];
-    uint32_t nb = *n_list;
-    if (nb > max_slots) nb = max_slots;
-    for (uint32_t bi = blockIdx.x; bi < nb; bi += gridDim.x) {
-        const uint64_t blk = list[bi];
-        uint8_t *slot = slots + (size_t)bi * sl.stride;
-        SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
-        const Record r = open_record(cv, blk);
-        bool ok = r.ok && !(hdr->bad[0] | hdr->bad[1] | hdr->bad[2]) && r.n_seq <= sl.ms;
-        Tokens t;
-        t.start = reinterpret_cast<uint16_t *>(slot + sl.o_start);
-        t.dst = reinterpret_cast<uint16_t *>(slot + sl.o_dst);
-        t.litpos = reinterpret_cast<uint16_t *>(slot + sl.o_litpos);
-        t.src = reinterpret_cast<uint64_t *>(slot + sl.o_src);
-        t.bm = nullptr;
-        if (ok) {
-            ok = parse_tokens(r, blk, slot + sl.o_len, slot + sl.o_off, t, warp_sums, nullptr);
-            if (!ok && threadIdx.x == 0) raise(ctl, kStTokens, blk);
-        }
-        if (threadIdx.x == 0) {
-            hdr->n_seq = r.n_seq;
-            hdr->n_lit = r.n_lit;
-            hdr->block_len = r.block_len;
-            hdr->parsed_ok = ok ? 1u : 0u;
-        }
-        __syncthreads();
     }
 }
 

@@ -2,137 +2,322 @@
 // ("a match referencing absolute position p can be resolved as soon as the block
 // containing p is available"; only the target block is written). SURVEY.md
 // section 8(c) reading A7: the paper does not say where a seeked block gets source bytes that
-// live in other blocks; here every needed position is followed, hop by hop, through the token
-// streams of the block that owns it until it lands on a literal.
+// live in other blocks; here every needed position is followed through the token streams of the
+// block that owns it until it lands on a literal.
 //
 // State: pend[i][o] = the absolute position whose byte value equals output byte o of target i
-// (initially the byte's own position), or kDone. One hop = collect the distinct blocks the
-// pending positions fall in -> entropy-decode + parse those blocks into slots -> resolve: a
-// position inside a literal run yields the byte; a position inside match k moves to
-// src_k + (o - dst_k), which is strictly smaller (src + len <= dst), so the chase terminates.
+// (initially the byte's own position), a literal request (slot + index into its LIT stream) once the
+// chase has reached a literal, or kDone. A position inside match k moves to src_k + (o - dst_k), which
+// is strictly smaller (src + len <= dst), so the chase terminates.
 #pragma once
 #include "match.cuh"
 
 namespace aceapex {
 
-constexpr uint32_t kChunk = 16;   // output bytes per thread in the per-byte kernels
+// ---------------------------------------------------------------------------------------------
+// Fused isolated decode: the whole hop loop in ONE kernel (north_star: "a fused single-block seek
+// path that does entropy decode, then gathers source bytes, then copies"). All CTAs are resident
+// (the host sizes the grid from the occupancy query), so the phases of a hop are separated by a
+// grid barrier instead of kernel boundaries, and the loop ends on the device when nothing is pending:
+// one launch per seek, no host read-back.
 
-__global__ void k_seek_init(Container cv, const uint64_t *ids, uint32_t n_targets, uint64_t *pend)
+// Grid barrier for co-resident CTAs: arrive on a counter, the last one opens the next generation.
+__device__ inline void grid_barrier(Control *ctl, uint32_t n_ctas)
 {
-    const uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;      // one thread per byte
-    if (g >= (uint64_t)n_targets * kB) return;
-    const uint32_t i = (uint32_t)(g >> kBlockLog2), o = (uint32_t)(g & (kB - 1));
-    const uint64_t id = ids[i];
-    pend[g] = (id < cv.n_blocks && o < block_len_of(cv, id)) ? (id << kBlockLog2) + o : kDone;
-}
-
-// Claim a slot for every distinct block that a pending position falls in.
-__global__ void k_seek_collect(const uint64_t *pend, uint64_t n_bytes, uint32_t *mark, uint32_t *slot_of,
-                               uint64_t *list, Control *ctl, uint32_t tag, uint32_t max_slots)
-{
-    const uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t g0 = c * kChunk;
-    if (g0 >= n_bytes) return;
-    uint64_t last = kDone;
-    for (uint32_t j = 0; j < kChunk; j++) {
-        const uint64_t p = pend[g0 + j];
-        if (p == kDone) continue;
-        const uint64_t blk = p >> kBlockLog2;
-        if (blk == last) continue;
-        last = blk;
-        if (mark[blk] == tag) continue;
-        if (atomicExch(mark + blk, tag) == tag) continue;     // somebody else claimed it
-        const uint32_t s = atomicAdd(&ctl->n_list, 1u);
-        slot_of[blk] = s;                                      // s >= max_slots: no slot this hop
-        if (s < max_slots) list[s] = blk;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const uint32_t gen = ld_acquire_u32(&ctl->bar_gen);
+        __threadfence();
+        if (atomicAdd(&ctl->bar_count, 1u) == n_ctas - 1) {
+            ctl->bar_count = 0;
+            __threadfence();
+            st_release_u32(&ctl->bar_gen, gen + 1);
+        } else {
+            while (ld_acquire_u32(&ctl->bar_gen) == gen) __nanosleep(40);
+        }
+        __threadfence();
     }
+    __syncthreads();
 }
 
-// Resolve every pending position whose block holds a slot in this hop.
-//   out mapping: packed -> target i at out + (out_base + i) * 16384; absolute -> out + ids[i] * 16384.
-__global__ void k_seek_resolve(Container cv, SlotLayout sl, const uint8_t *slots, uint64_t *pend,
-                               uint32_t n_targets, const uint64_t *ids, const uint32_t *mark,
-                               const uint32_t *slot_of, Control *ctl, uint32_t tag, uint32_t max_slots,
-                               uint8_t *out, uint64_t out_base, uint32_t absolute)
+// Parse the decoded LEN / OFF streams of the block in `slot` into the slot's token arrays, by ONE warp
+// (FORMAT.md section 4; same rules as the match kernel's parse, restated for a warp: 32 sequences per
+// round, one packed warp scan, carries in registers). Sets hdr->parsed_ok.
+__device__ inline void warp_parse_block(const Container &cv, const SlotLayout &sl, uint8_t *slot, uint64_t blk,
+                                        Control *ctl, uint32_t lane)
 {
-    const uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t g0 = c * kChunk;
-    uint32_t remaining = 0;
-    if (g0 < (uint64_t)n_targets * kB) {
-        const uint32_t i = (uint32_t)(g0 >> kBlockLog2);
-        uint8_t *dst = out + ((absolute ? ids[i] : out_base + i) << kBlockLog2) + (g0 & (kB - 1));
-        // cache of the sequence found for the previous byte
-        uint64_t c_blk = kDone;
-        const uint8_t *c_slot = nullptr;
-        uint32_t c_q = 0, c_lo = 1, c_hi = 0, c_nseq = 0, c_blen = 0;
-        const uint16_t *c_start = nullptr;
-        for (uint32_t j = 0; j < kChunk; j++) {
-            const uint64_t p = pend[g0 + j];
-            if (p == kDone) continue;
-            const uint64_t blk = p >> kBlockLog2;
-            const uint32_t o = (uint32_t)(p & (kB - 1));
-            if (blk != c_blk) {
-                c_blk = blk;
-                c_slot = nullptr;
-                c_lo = 1; c_hi = 0;
-                if (mark[blk] == tag) {
-                    const uint32_t s = slot_of[blk];
-                    if (s < max_slots) {
-                        c_slot = slots + (size_t)s * sl.stride;
-                        const SlotHdr *h = reinterpret_cast<const SlotHdr *>(c_slot + sl.o_hdr);
-                        if (!h->parsed_ok) {
-                            c_slot = nullptr;
-                            c_blk = kDone;
-                            pend[g0 + j] = kDone;              // corrupt block: give up on this byte
-                            raise(ctl, kStChase, blk);
-                            continue;
-                        }
-                        c_nseq = h->n_seq;
-                        c_blen = h->block_len;
-                        c_start = reinterpret_cast<const uint16_t *>(c_slot + sl.o_start);
-                    }
-                }
+    SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
+    bool ok = !(hdr->bad[LEN] | hdr->bad[OFF]);                        // the LIT stream is decoded later, on demand
+    const uint32_t n = hdr->n_seq, n_lit = hdr->n_lit, blen = hdr->block_len, n_extras = hdr->n_extras;
+    const uint32_t onb = hdr->off_nbytes;
+    ok = ok && n <= sl.ms && onb >= 1 && onb <= 8;
+    if (ok) {
+        const uint16_t *len16 = reinterpret_cast<const uint16_t *>(slot + sl.o_len);
+        const uint8_t *off_s = slot + sl.o_off;
+        const uint16_t *extras = reinterpret_cast<const uint16_t *>(cv.payload + ((uint64_t)hdr->rec_lo | (uint64_t)hdr->rec_hi << 32) +
+                                                                    hdr->extras_off);
+        uint16_t *start = reinterpret_cast<uint16_t *>(slot + sl.o_start);
+        uint16_t *dst = reinterpret_cast<uint16_t *>(slot + sl.o_dst);
+        uint16_t *litpos = reinterpret_cast<uint16_t *>(slot + sl.o_litpos);
+        uint64_t *srcv = reinterpret_cast<uint64_t *>(slot + sl.o_src);
+        const uint64_t B0 = blk << kBlockLog2;
+        uint32_t lp = 0, pos = 0, e = 0;                               // warp-uniform carries
+        bool bad = false;
+        const uint64_t src_mask = ~0ull >> (64 - 8 * onb);
+        // loads of round i+1 are issued before round i is processed (one warp: latency is everything)
+        uint32_t v_nx = 0, w0_nx = 0, w1_nx = 0, w2_nx = 0;
+        auto fetch = [&](uint32_t k) {
+            v_nx = w0_nx = w1_nx = w2_nx = 0;
+            if (k < n) {
+                v_nx = len16[k];
+                const uint32_t *wp = reinterpret_cast<const uint32_t *>(off_s + ((k * onb) & ~3u));   // stays inside the slot
+                w0_nx = wp[0]; w1_nx = wp[1]; w2_nx = wp[2];
             }
-            if (!c_slot) { remaining++; continue; }            // no slot this hop: try again next hop
-            if (o >= c_blen) { pend[g0 + j] = kDone; raise(ctl, kStChase, blk); continue; }
-            if (!(o >= c_lo && o < c_hi)) {
-                // largest q in [0, n_seq] with start[q] <= o (start[0] == 0)
-                uint32_t lo = 0, hi = c_nseq;
-                while (lo < hi) {
-                    const uint32_t mid = (lo + hi + 1) >> 1;
-                    if (c_start[mid] <= o) lo = mid; else hi = mid - 1;
-                }
-                c_q = lo;
-                c_lo = c_start[lo];
-                c_hi = lo < c_nseq ? c_start[lo + 1] : c_blen;
+        };
+        fetch(lane);
+        for (uint32_t kb = 0; kb < n; kb += 32) {
+            const uint32_t k = kb + lane;
+            const bool act = k < n;
+            const uint32_t v = v_nx, w0 = w0_nx, w1 = w1_nx, w2 = w2_nx;
+            fetch(k + 32);
+            uint32_t ll = 0, ml = 0;
+            if (act) { ll = v & 0xFFu; ml = (v >> 8) + 4; }
+            if (n_extras) {                                            // warp-uniform: escapes are rare
+                const uint32_t e_ll = ll == 255, e_ml = ml == 259;
+                uint32_t etot;
+                uint32_t ei = e + warp_excl_scan(e_ll + e_ml, lane, etot);
+                e += etot;
+                if (e > n_extras) { bad = true; break; }               // warp-uniform
+                if (e_ll) ll = extras[ei++];
+                if (e_ml) ml = (uint32_t)extras[ei] + 4;
+            } else if (ll == 255 || ml == 259) {
+                bad = true;                                            // an escape without extras
             }
-            const uint32_t q = c_q;
-            const uint32_t d = q < c_nseq ? reinterpret_cast<const uint16_t *>(c_slot + sl.o_dst)[q] : c_blen;
-            if (o < d) {                                       // a literal: the origin
-                const uint32_t lp = reinterpret_cast<const uint16_t *>(c_slot + sl.o_litpos)[q];
-                dst[j] = c_slot[sl.o_lit + lp + (o - c_lo)];
-                pend[g0 + j] = kDone;
-            } else {                                           // a match: follow the absolute offset
-                const uint64_t nxt = reinterpret_cast<const uint64_t *>(c_slot + sl.o_src)[q] + (o - d);
-                if (nxt >= p) { pend[g0 + j] = kDone; raise(ctl, kStChase, blk); continue; }
-                pend[g0 + j] = nxt;
-                remaining++;
+            // an invalid stream may overflow 16 bits, so the two running sums are scanned apart
+            uint32_t t_ll, t_all;
+            const uint32_t p_ll = warp_excl_scan(ll, lane, t_ll), p_all = warp_excl_scan(ll + ml, lane, t_all);
+            const uint32_t my_lp = lp + p_ll, my_st = pos + p_all;
+            lp += t_ll; pos += t_all;
+            if (lp > n_lit || pos > blen) { bad = true; break; }       // warp-uniform; bounds every value below
+            if (act) {
+                const uint32_t sh = ((k * onb) & 3u) * 8;
+                const uint32_t lo = __funnelshift_r(w0, w1, sh), hi = __funnelshift_r(w1, w2, sh);
+                const uint64_t src = (((uint64_t)hi << 32) | lo) & src_mask;
+                start[k] = (uint16_t)my_st;
+                litpos[k] = (uint16_t)my_lp;
+                dst[k] = (uint16_t)(my_st + ll);
+                srcv[k] = src;
+                if (src + ml > B0 + my_st + ll) bad = true;            // strictly before, non-overlapping
             }
         }
+        bad = __any_sync(0xFFFFFFFFu, bad);
+        if (!bad) bad = e != n_extras || pos + (n_lit - lp) != blen;
+        if (!bad && lane == 0) { start[n] = (uint16_t)pos; litpos[n] = (uint16_t)lp; }
+        ok = !bad;
+        if (!ok && lane == 0) raise(ctl, kStTokens, blk);
     }
-    // CTA-level count of what is still pending
-    __shared__ uint32_t s_rem;
-    if (threadIdx.x == 0) s_rem = 0;
-    __syncthreads();
-    if (remaining) atomicAdd(&s_rem, remaining);
-    __syncthreads();
-    if (threadIdx.x == 0 && s_rem) atomicAdd(&ctl->pending, (unsigned long long)s_rem);
+    if (lane == 0) hdr->parsed_ok = ok ? 1u : 0u;
+    __syncwarp();
 }
 
-// After the promised number of hops nothing may be pending (header promise D, FORMAT.md section 1).
-__global__ void k_seek_check(Control *ctl)
+struct SeekArgs {
+    uint64_t *pend;          // [nt][16384] per target byte: kDone | literal request | absolute position being chased
+    uint32_t *mark, *slot_of;
+    uint64_t *list;
+    const uint64_t *ids;     // nt target ids (device); nullptr: the single target `one_id`
+    uint64_t one_id;
+    uint8_t *slots;
+    uint8_t *out;
+    uint64_t out_base;       // packed mode: target i lands at out + (out_base + i) * 16384
+    uint32_t nt, absolute, max_slots;
+    uint32_t tag0;           // round r marks the blocks it claims with tag0 + r
+    uint32_t max_hops;
+};
+
+constexpr unsigned long long kLitReq = 1ull << 62;   // pend = kLitReq | slot << 14 | index into the slot's LIT stream
+
+__device__ inline uint64_t seek_target(const SeekArgs &a, uint32_t i) { return a.ids ? a.ids[i] : a.one_id; }
+
+// Follow one byte through the parsed blocks that hold a slot in this round (mark == tag, slot index
+// below n_slots_ready) until it reaches a literal (-> literal request), leaves the resident set
+// (-> stays a position, claimed by the next hop's collect) or hits an inconsistency (-> kDone + status).
+__device__ inline unsigned long long chase_byte(const SlotLayout &sl, const SeekArgs &a, Control *ctl, uint32_t tag,
+                                                uint32_t n_ready, unsigned long long p)
 {
-    if (ctl->pending != 0) raise(ctl, kStChase, 0);
+    for (;;) {
+        const uint64_t blk = p >> kBlockLog2;
+        const uint32_t o = (uint32_t)(p & (kB - 1));
+        if (a.mark[blk] != tag) return p;
+        const uint32_t s = a.slot_of[blk];
+        if (s >= n_ready) return p;                                    // claimed, but no slot in this round
+        uint8_t *slot = a.slots + (size_t)s * sl.stride;
+        SlotHdr *h = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
+        if (!h->parsed_ok) { raise(ctl, kStChase, blk); return kDone; }   // corrupt block: give up on this byte
+        const uint32_t n = h->n_seq, blen = h->block_len;
+        if (o >= blen) { raise(ctl, kStChase, blk); return kDone; }
+        const uint16_t *start = reinterpret_cast<const uint16_t *>(slot + sl.o_start);
+        uint32_t lo = 0, hi = n;                                       // largest q in [0, n] with start[q] <= o
+        while (lo < hi) {
+            const uint32_t mid = (lo + hi + 1) >> 1;
+            if (start[mid] <= o) lo = mid; else hi = mid - 1;
+        }
+        const uint32_t q = lo, st = start[q];
+        const uint32_t d = q < n ? reinterpret_cast<const uint16_t *>(slot + sl.o_dst)[q] : blen;
+        if (o < d) {                                                   // a literal: the origin
+            const uint32_t li = (uint32_t)reinterpret_cast<const uint16_t *>(slot + sl.o_litpos)[q] + (o - st);
+            if (li >= kB) { raise(ctl, kStChase, blk); return kDone; }
+            h->need_lit = 1;
+            return kLitReq | (unsigned long long)s << kBlockLog2 | li;
+        }
+        const unsigned long long nxt = reinterpret_cast<const uint64_t *>(slot + sl.o_src)[q] + (o - d);   // a match
+        if (nxt >= p) { raise(ctl, kStChase, blk); return kDone; }
+        p = nxt;
+    }
+}
+
+// The fused kernel. CTAs of kEntropyWarps warps (the entropy phases need the per-warp tables), all
+// co-resident. A ROUND keeps every block it touches resident in a slot:
+//   chase hops:  collect the blocks of the bytes still chasing -> entropy-decode the LEN and OFF streams
+//                of the NEW blocks (short streams) -> parse them -> follow every byte through all resident
+//                blocks until it lands on a literal (a literal request: slot + index) or leaves them;
+//   until nothing is chasing (or the slots are used up); then ONE literal phase:
+//   entropy-decode the LIT stream of the slots that received a literal request, deliver the bytes.
+// A seek therefore pays for the long LIT streams once, not once per hop, and ends on the device.
+__global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv, SlotLayout sl, SeekArgs a, Control *ctl)
+{
+    extern __shared__ __align__(1024) uint8_t smem_entropy[];
+    __shared__ uint32_t s_rem;
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    WarpSmem ws;
+    {
+        const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(smem_entropy);
+        const uint32_t pad = (0u - a0) & (kT8Bytes - 1);
+        uint8_t *base = smem_entropy + pad;
+        ws.t8 = base + warp * kT8Bytes;
+        ws.syml = reinterpret_cast<uint2 *>(base + kEntropyWarps * kT8Bytes + warp * kSymlBytes);
+        ws.ring = base + kEntropyWarps * (kT8Bytes + kSymlBytes) + warp * kRingBytes;
+        ws.a_t8 = (uint32_t)__cvta_generic_to_shared(ws.t8);
+        ws.a_syml = (uint32_t)__cvta_generic_to_shared(ws.syml);
+        ws.a_ring = (uint32_t)__cvta_generic_to_shared(ws.ring);
+    }
+    const uint32_t n_ctas = gridDim.x;
+    const uint64_t n_thr = (uint64_t)n_ctas * blockDim.x, gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t n_warps = n_ctas * kEntropyWarps, gwarp = blockIdx.x * kEntropyWarps + warp;
+    const uint64_t n_bytes = (uint64_t)a.nt * kB;
+#ifdef ACEAPEX_TRACE
+    long long st_prev = clock64();
+#define SEEK_MARK(i) do { if (gtid == 0) { const long long t_ = clock64(); atomicAdd(&g_trace[i], (unsigned long long)(t_ - st_prev)); st_prev = t_; } } while (0)
+#else
+#define SEEK_MARK(i) do { } while (0)
+#endif
+
+    // init: every target byte chases its own position
+    for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
+        const uint64_t id = seek_target(a, (uint32_t)(g >> kBlockLog2));
+        const uint32_t o = (uint32_t)(g & (kB - 1));
+        a.pend[g] = (id < cv.n_blocks && o < block_len_of(cv, id)) ? (id << kBlockLog2) + o : kDone;
+    }
+    grid_barrier(ctl, n_ctas);
+
+    uint32_t hop = 0;
+    for (uint32_t round = 0;; round++) {
+        const uint32_t rp = round & 1u, tag = a.tag0 + round;
+        uint32_t n_ready = 0;                                          // slots of this round decoded and parsed
+        unsigned long long chasing = 0;
+        for (;; hop++) {
+            const uint32_t hp = hop & 1u;
+            SEEK_MARK(10);
+            // ---- collect: claim a slot for every distinct block a chasing byte sits in
+            for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
+                const uint64_t p = a.pend[g];
+                if (p >= kLitReq) continue;                            // done, or waiting for its literal
+                const uint64_t blk = p >> kBlockLog2;
+                if (a.mark[blk] == tag) continue;
+                if (atomicExch(a.mark + blk, tag) == tag) continue;    // somebody else claimed it
+                const uint32_t s = atomicAdd(&ctl->round_n_list[rp], 1u);
+                a.slot_of[blk] = s;                                    // s >= max_slots: no slot in this round
+                if (s < a.max_slots) a.list[s] = blk;
+            }
+            grid_barrier(ctl, n_ctas);
+            if (gtid == 0) {                                           // the other parities' counters are idle now
+                ctl->hop_pending[hp ^ 1u] = 0;
+                if (n_ready == 0) ctl->round_n_list[rp ^ 1u] = 0;
+            }
+            const uint32_t n_claimed = ctl->round_n_list[rp];
+            const uint32_t n_now = n_claimed < a.max_slots ? n_claimed : a.max_slots;
+            SEEK_MARK(11);
+#ifdef ACEAPEX_TRACE
+            if (gtid == 0) atomicAdd(&g_trace[15], 1ull);
+#endif
+            // ---- entropy: LEN and OFF of the new blocks, warp per (block, stream) unit
+            const uint32_t n_new = n_now - n_ready;
+            for (uint32_t u = gwarp; u < 2 * n_new; u += n_warps) {
+                const uint32_t so = u / n_new, bi = n_ready + (u - so * n_new);
+                if (so == 1 && lane == 0) reinterpret_cast<SlotHdr *>(a.slots + (size_t)bi * sl.stride + sl.o_hdr)->need_lit = 0;
+                decode_unit(cv, sl, a.slots, a.list[bi], bi, so == 0 ? OFF : LEN, so == 1, ws, lane, ctl);
+            }
+            grid_barrier(ctl, n_ctas);
+            SEEK_MARK(12);
+            // ---- parse the new blocks, warp per block
+            for (uint32_t bi = n_ready + gwarp; bi < n_now; bi += n_warps)
+                warp_parse_block(cv, sl, a.slots + (size_t)bi * sl.stride, a.list[bi], ctl, lane);
+            grid_barrier(ctl, n_ctas);
+            SEEK_MARK(13);
+            n_ready = n_now;
+            // ---- chase every byte through the resident blocks
+            if (threadIdx.x == 0) s_rem = 0;
+            __syncthreads();
+            uint32_t remaining = 0;
+            for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
+                const unsigned long long p = a.pend[g];
+                if (p >= kLitReq) continue;
+                const unsigned long long q = chase_byte(sl, a, ctl, tag, n_ready, p);
+                if (q != p) a.pend[g] = q;
+                remaining += q < kLitReq;
+            }
+            remaining = __reduce_add_sync(0xFFFFFFFFu, remaining);
+            if (lane == 0 && remaining) atomicAdd(&s_rem, remaining);
+            __syncthreads();
+            if (threadIdx.x == 0 && s_rem) atomicAdd(&ctl->hop_pending[hp], (unsigned long long)s_rem);
+            grid_barrier(ctl, n_ctas);
+            chasing = ctl->hop_pending[hp];
+            SEEK_MARK(14);
+            if (chasing == 0 || n_claimed >= a.max_slots || hop + 1 >= a.max_hops) { hop++; break; }
+        }
+        // ---- literal phase: LIT stream of every slot with a request, then deliver
+        for (uint32_t bi = gwarp; bi < n_ready; bi += n_warps) {
+            const SlotHdr *h = reinterpret_cast<const SlotHdr *>(a.slots + (size_t)bi * sl.stride + sl.o_hdr);
+            if (h->need_lit && h->parsed_ok) decode_unit(cv, sl, a.slots, a.list[bi], bi, LIT, false, ws, lane, ctl);
+        }
+        grid_barrier(ctl, n_ctas);
+        SEEK_MARK(8);
+        for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
+            const unsigned long long p = a.pend[g];
+            if (p == kDone || p < kLitReq) continue;
+            const uint32_t s = (uint32_t)((p ^ kLitReq) >> kBlockLog2), li = (uint32_t)(p & (kB - 1));
+            const uint8_t *slot = a.slots + (size_t)s * sl.stride;
+            const SlotHdr *h = reinterpret_cast<const SlotHdr *>(slot + sl.o_hdr);
+            if (!h->bad[LIT] && li < h->n_lit) {
+                const uint32_t i = (uint32_t)(g >> kBlockLog2);
+                a.out[((a.absolute ? seek_target(a, i) : a.out_base + i) << kBlockLog2) + (g & (kB - 1))] = slot[sl.o_lit + li];
+            } else {
+                raise(ctl, kStChase, a.list[s]);
+            }
+            a.pend[g] = kDone;
+        }
+        if (chasing == 0) break;
+        if (hop >= a.max_hops) {                                       // deeper than this build follows a chain
+            if (gtid == 0) raise(ctl, kStChase, 0);
+            break;
+        }
+        grid_barrier(ctl, n_ctas);                                     // the slots are recycled by the next round
+    }
+    // leave the counters of both parities at zero for the next call
+    grid_barrier(ctl, n_ctas);
+    if (gtid == 0) {
+        ctl->round_n_list[0] = ctl->round_n_list[1] = 0;
+        ctl->hop_pending[0] = ctl->hop_pending[1] = 0;
+    }
 }
 
 }  // namespace aceapex
