@@ -70,12 +70,17 @@ typedef struct {
     uint32_t threads;      /* worker threads for the parse (result does not depend on it) */
     uint32_t batch;        /* blocks parsed against one snapshot of the global table when R > 0
                               (default 64; part of the encoder's definition, not of the format) */
+    uint32_t raw_slack_pct; /* selective entropy (FORMAT.md section 2 "modes"): a stream is stored
+                              RAW when n_sym * 100 <= (tbl_bytes + 2 * n_words) * (100 + raw_slack_pct), i.e.
+                              when rANS saves less than that margin. Default 0: RAW only where rANS does not
+                              shrink the stream. 0xFFFFFFFF: never RAW. */
 } ora_enc_params;
 
 typedef struct {
     uint64_t n_seq, n_lit, match_bytes, intra_match_bytes, n_extras;
     uint64_t n_sym[3], n_words[3], table_bytes;
     uint32_t max_depth_seen, max_level_seen;
+    uint64_t n_raw[3];     /* streams stored RAW, per stream id */
 } ora_enc_stats;
 
 void ora_enc_params_default(ora_enc_params *p);

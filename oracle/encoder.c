@@ -74,6 +74,7 @@ void ora_enc_params_default(ora_enc_params *p)
     p->offset_width = 4;
     p->threads = 1;
     p->batch = 64;
+    p->raw_slack_pct = 0;
 }
 
 size_t ora_encode_bound(size_t n)
@@ -241,6 +242,7 @@ static int serialise_block(const enc_ctx *e, uint64_t b, enc_scratch *s, uint32_
     uint8_t tables[3][32 + 512];
     uint32_t tbl_bytes[3] = { 0, 0, 0 };
     size_t n_words[3] = { 0, 0, 0 };
+    uint32_t modes = 0;
     for (int k = 0; k < 3; k++) {
         uint32_t count[256] = { 0 };
         uint16_t freq[256];
@@ -249,6 +251,20 @@ static int serialise_block(const enc_ctx *e, uint64_t b, enc_scratch *s, uint32_
         int rc = ora_rans_encode(sym[k], n_sym[k], freq, 32, out->states[k], s->words[k], &n_words[k]);
         if (rc != ORA_OK) return rc;
         if (n_sym[k]) tbl_bytes[k] = table_write(tables[k], freq);
+        /* selective entropy ("apply ANS selectively"; FORMAT.md section 2 modes): keep the
+         * stream verbatim when rANS does not pay for itself */
+        if (n_sym[k] && e->p.raw_slack_pct != 0xFFFFFFFFu &&
+            (uint64_t)n_sym[k] * 100 <= ((uint64_t)tbl_bytes[k] + 2 * (uint64_t)n_words[k]) * (100 + (uint64_t)e->p.raw_slack_pct)) {
+            modes |= 1u << (2 * k);
+            tbl_bytes[k] = 0;
+            n_words[k] = (n_sym[k] + 1) / 2;
+            for (uint32_t i = 0; i < n_words[k]; i++) {
+                uint32_t lo = sym[k][2 * i], hi = 2 * i + 1 < n_sym[k] ? sym[k][2 * i + 1] : 0;
+                s->words[k][i] = (uint16_t)(lo | hi << 8);            /* bytes in order, little-endian words */
+            }
+            for (int l = 0; l < 32; l++) out->states[k][l] = 65536u;
+            out->st.n_raw[k]++;
+        }
     }
     size_t pos = ORA_REC_HDR_BYTES;
     for (int k = 0; k < 3; k++) pos = pad16(pos) + tbl_bytes[k];
@@ -259,7 +275,7 @@ static int serialise_block(const enc_ctx *e, uint64_t b, enc_scratch *s, uint32_
     uint8_t *rec = (uint8_t *)calloc(rec_bytes, 1);
     if (!rec) return ORA_E_NOMEM;
     wr16(rec + 0, n_seq); wr16(rec + 2, n_lit); wr16(rec + 4, n_extras);
-    rec[6] = (uint8_t)off_nbytes; rec[7] = 0;
+    rec[6] = (uint8_t)off_nbytes; rec[7] = (uint8_t)modes;
     for (int k = 0; k < 3; k++) { wr32(rec + 8 + 4 * k, (uint32_t)n_words[k]); wr16(rec + 20 + 2 * k, tbl_bytes[k]); }
     pos = ORA_REC_HDR_BYTES;
     for (int k = 0; k < 3; k++) { pos = pad16(pos); memcpy(rec + pos, tables[k], tbl_bytes[k]); pos += tbl_bytes[k]; }
@@ -369,7 +385,7 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *pp, uint8_t *o
             const ora_enc_stats *t = &blocks[b].st;
             S.n_seq += t->n_seq; S.n_lit += t->n_lit; S.match_bytes += t->match_bytes;
             S.intra_match_bytes += t->intra_match_bytes; S.n_extras += t->n_extras; S.table_bytes += t->table_bytes;
-            for (int k = 0; k < 3; k++) { S.n_sym[k] += t->n_sym[k]; S.n_words[k] += t->n_words[k]; }
+            for (int k = 0; k < 3; k++) { S.n_sym[k] += t->n_sym[k]; S.n_words[k] += t->n_words[k]; S.n_raw[k] += t->n_raw[k]; }
             if (t->max_depth_seen > S.max_depth_seen) S.max_depth_seen = t->max_depth_seen;
             if (t->max_level_seen > S.max_level_seen) S.max_level_seen = t->max_level_seen;
         }

@@ -246,6 +246,20 @@ __device__ inline bool decode_stream(uint32_t x /* this lane's initial state */,
     return __all_sync(0xFFFFFFFFu, x == kRansL) && wpos2 == wbytes;
 }
 
+// A RAW stream (FORMAT.md section 2, mode 1): the symbols are stored verbatim in the words
+// section. Both ends are 16-byte aligned and padded inside their areas, so the warp copies whole uint4s.
+// The unused rANS states must be 2^16 and the pad byte of an odd-length stream 0.
+__device__ inline bool copy_raw_stream(uint32_t x, uint32_t n, const uint8_t *words_sec, uint8_t *out, uint32_t lane)
+{
+    bool ok = x == kRansL;
+    const uint4 *src = reinterpret_cast<const uint4 *>(words_sec);
+    uint4 *dst = reinterpret_cast<uint4 *>(out);
+    const uint32_t nv = (n + 15) >> 4;
+    for (uint32_t i = lane; i < nv; i += 32) dst[i] = src[i];
+    if ((n & 1u) && lane == 0 && words_sec[n] != 0) ok = false;
+    return __all_sync(0xFFFFFFFFu, ok);
+}
+
 // One (block, stream) unit, by one warp: stream s of block blk into slot bi. Output: the slot's stream
 // area and bad flag; with write_hdr also the record header fields in the slot header.
 __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, uint8_t *slots, uint64_t blk, uint32_t bi,
@@ -277,7 +291,9 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
         const uint32_t tb = s == LIT ? r.tbl_bytes[LIT] : (s == LEN ? r.tbl_bytes[LEN] : r.tbl_bytes[OFF]);
         const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
         const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
-        ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
+        const uint32_t is_raw = s == LIT ? r.raw[LIT] : (s == LEN ? r.raw[LEN] : r.raw[OFF]);
+        if (is_raw) ok = copy_raw_stream(x0, n, r.rec + wo, out, lane);
+        else ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
         if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
     } else if (lane == 0) {
         raise(ctl, kStRecord, blk);

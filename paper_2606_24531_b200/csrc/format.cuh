@@ -37,6 +37,7 @@ struct Record {
     const uint8_t *rec;
     uint32_t block_len, n_seq, n_lit, n_extras, off_nbytes;
     uint32_t n_sym[3], n_words[3], tbl_bytes[3];
+    uint32_t raw[3];           // stream stored RAW (FORMAT.md section 2 modes; PAPER.md:94 selective entropy)
     uint32_t tbl_off[3], extras_off, tags_off, words_off[3];
     bool ok;
 };
@@ -58,7 +59,7 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
     r.rec = nullptr;
     r.block_len = block_len_of(cv, b);
     r.n_seq = r.n_lit = r.n_extras = r.off_nbytes = 0;
-    for (int s = 0; s < 3; s++) { r.n_sym[s] = r.n_words[s] = r.tbl_bytes[s] = r.tbl_off[s] = r.words_off[s] = 0; }
+    for (int s = 0; s < 3; s++) { r.n_sym[s] = r.n_words[s] = r.tbl_bytes[s] = r.tbl_off[s] = r.words_off[s] = r.raw[s] = 0; }
     r.extras_off = r.tags_off = 0;
     const uint64_t o0 = cv.rec_off[b], o1 = cv.rec_off[b + 1];
     if (o1 < o0 || (o0 & 15) || (o1 & 15) || o1 - o0 < kRecHeaderBytes || o1 > cv.payload_bytes) return r;
@@ -81,7 +82,8 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
     r.tbl_bytes[OFF] = h1.z & 0xFFFFu;
     if (r.n_seq > kMaxSeq || r.n_lit > r.block_len) return r;
     if (r.off_nbytes < 1 || r.off_nbytes > cv.W) return r;
-    if (modes != 0) return r;                          // only rANS mode in version 1
+    if (modes & ~0x15u) return r;                      // per stream: 0 = rANS, 1 = RAW; everything else reserved
+    r.raw[LIT] = modes & 1u; r.raw[LEN] = (modes >> 2) & 1u; r.raw[OFF] = (modes >> 4) & 1u;
     if (r.n_extras > 2 * r.n_seq) return r;
     r.n_sym[LIT] = r.n_lit;
     r.n_sym[LEN] = 2 * r.n_seq;
@@ -92,8 +94,12 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
         r.tbl_off[s] = pos;
         if (r.tbl_bytes[s] > 32 + 512) return r;
         pos += r.tbl_bytes[s];
-        if ((r.n_sym[s] == 0) != (r.tbl_bytes[s] == 0)) return r;
-        if (r.n_words[s] > r.n_sym[s]) return r;
+        if (r.raw[s]) {                                // no table; the symbols sit in the words section
+            if (r.n_sym[s] == 0 || r.tbl_bytes[s] != 0 || r.n_words[s] != (r.n_sym[s] + 1) / 2) return r;
+        } else {
+            if ((r.n_sym[s] == 0) != (r.tbl_bytes[s] == 0)) return r;
+            if (r.n_words[s] > r.n_sym[s]) return r;
+        }
     }
     pos = pad16(pos); r.extras_off = pos; pos += 2 * r.n_extras;
     pos = pad16(pos); r.tags_off = pos; pos += (r.n_seq + 1) / 2;

@@ -58,8 +58,16 @@ def compute_tags(block_start, seqs):
     return tags
 
 
-def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off_nbytes=None, freqs=None):
-    """seqs: list of (lit_len, match_len, src). `literals`: all literal bytes of the block."""
+def _raw_stream(sym: bytes):
+    """FORMAT.md section 2, mode 1 (RAW): no table, the symbols verbatim in the words section."""
+    assert len(sym) >= 1
+    body = bytes(sym) + (b"\0" if len(sym) & 1 else b"")
+    return b"", body, len(body) // 2, [65536] * 32
+
+
+def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off_nbytes=None, freqs=None, raw=()):
+    """seqs: list of (lit_len, match_len, src). `literals`: all literal bytes of the block.
+    raw: names of the streams ("lit", "len", "off") to store RAW instead of rANS-coded."""
     if tags is None:
         tags = compute_tags(block_start, seqs)
     if off_nbytes is None:
@@ -78,9 +86,10 @@ def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off
             extras.append(ml - 4)
         off_sym += int(src).to_bytes(8, "little")[:off_nbytes]
     freqs = freqs or {}
-    streams = [_stream(bytes(literals), freqs.get("lit")), _stream(bytes(len_sym), freqs.get("len")),
-               _stream(bytes(off_sym), freqs.get("off"))]
-    hdr = struct.pack("<HHHBB", len(seqs), len(literals), len(extras), off_nbytes, 0)
+    syms = {"lit": bytes(literals), "len": bytes(len_sym), "off": bytes(off_sym)}
+    streams = [_raw_stream(syms[k]) if k in raw else _stream(syms[k], freqs.get(k)) for k in ("lit", "len", "off")]
+    modes = sum(1 << (2 * i) for i, k in enumerate(("lit", "len", "off")) if k in raw)
+    hdr = struct.pack("<HHHBB", len(seqs), len(literals), len(extras), off_nbytes, modes)
     hdr += struct.pack("<III", *(s[2] for s in streams))
     hdr += struct.pack("<HHH", *(len(s[0]) for s in streams))
     hdr += b"\0" * 6

@@ -14,7 +14,7 @@ import pytest
 import oracle
 from paper_2606_24531_b200 import workloads as W
 
-from handmade import B, build_container, build_record, container_from_tokens
+from handmade import B, build_container, build_record, container_from_tokens, expand
 from test_oracle_codec import ADVERSARIAL, handmade_case
 
 torch = pytest.importorskip("torch")
@@ -340,3 +340,45 @@ def test_broken_depth_promise_does_not_affect_isolated_decode(binding):
             dec.check()
             blk = iso.decode(b)
             assert np.array_equal(got[:blk.size], blk)
+
+
+# ---- selective entropy: RAW streams (FORMAT.md section 2 modes)
+
+def test_raw_streams_handmade_and_encoder_chosen(binding):
+    total, blocks = handmade_case()
+    want = np.frombuffer(expand(total, blocks), np.uint8)
+    for raw in [("lit",), ("len",), ("off",), ("lit", "len", "off")]:
+        recs = []
+        for b, (seqs, lits) in enumerate(blocks):
+            use = tuple(k for k in raw if not (k == "lit" and len(lits) == 0))
+            recs.append(build_record(b * B, seqs, lits, raw=use))
+        full_check(binding, build_container(total, recs), want, n_targets=2)
+    # encoder-chosen: uniform random bytes (LIT raw in every block) and a high slack (everything raw)
+    rnd = W.generate("random", 5 * B + 77, 11)
+    c, st = oracle.encode(rnd, return_stats=True)
+    assert st.n_raw[0] == 6
+    full_check(binding, c, rnd, n_targets=3)
+    fq = W.generate("fastq", 24 * B + 5, 12)
+    c, st = oracle.encode(fq, return_stats=True, min_match=8, max_depth=8, window=4, batch=4, raw_slack_pct=1000)
+    assert sum(st.n_raw) >= 2 * 25
+    full_check(binding, c, fq, n_targets=5, seek_blocks=[0, 24, 7, 19, 13, 3])
+
+
+def test_rejects_inconsistent_raw_streams(binding):
+    total, blocks = handmade_case()
+    recs = [build_record(b * B, s, l, raw=("len",)) for b, (s, l) in enumerate(blocks)]
+    good = build_container(total, recs)
+    i = oracle.info(good)
+    bad = good.copy(); bad[i.payload_off + 7] = 0x08                      # reserved mode 2 for LEN
+    assert open_rc(binding, bad) == binding.E_CORRUPT
+    bad = good.copy(); bad[i.payload_off + 8 + 4] ^= 1                    # n_words[LEN] != ceil(n_sym / 2)
+    assert open_rc(binding, bad) == binding.E_CORRUPT
+    bad = good.copy()
+    st = 64 + (i.n_blocks + 1) * 8 + (1 * 3 + 1) * 32 * 4 + 7 * 4         # block 1, LEN stream, lane 7
+    bad[st] ^= 1                                                          # an unused state that is not 2^16
+    expect_corrupt(binding, bad, total, 1)
+    rec, stt = build_record(0, [], b"abc", raw=("lit",))
+    c = build_container(3, [(rec, stt)])
+    full_check(binding, c, np.frombuffer(b"abc", np.uint8), n_targets=1)
+    bad = c.copy(); bad[oracle.info(c).payload_off + 32 + 3] = 1          # pad byte of the odd raw stream
+    expect_corrupt(binding, bad, 3, 0)

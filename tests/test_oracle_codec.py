@@ -233,3 +233,81 @@ def test_validator_flags_wrong_tags_and_broken_promises():
     with pytest.raises(oracle.OracleError) as e:     # window promise: block 2 reads block 1
         oracle.validate(build_container(total, recs, window=2))
     assert e.value.code == -7
+
+
+# ---- selective entropy: RAW streams (FORMAT.md section 2 modes)
+
+def test_raw_streams_decode_to_plain_definition():
+    """Hand-written records whose streams are stored RAW (no rANS involved at all for the raw ones):
+    the decoded bytes are known by construction, for every combination of raw / coded streams."""
+    total, blocks = handmade_case()
+    want = expand(total, blocks)
+    for raw in [("lit",), ("len",), ("off",), ("lit", "len", "off"), ("len", "off")]:
+        recs = []
+        for b, (seqs, lits) in enumerate(blocks):
+            use = tuple(k for k in raw if not (k == "lit" and len(lits) == 0))   # an empty stream cannot be RAW
+            recs.append(build_record(b * B, seqs, lits, raw=use))
+        c = build_container(total, recs)
+        assert oracle.decode_all(c).tobytes() == want, raw
+        with oracle.Isolated(c) as iso:
+            for b in range(3):
+                assert iso.decode(b).tobytes() == want[b * B:(b + 1) * B]
+        assert oracle.validate(c).n_matches_spanning == 1
+        h, lit, ln, off, ex, tg = oracle.decode_streams(c, 1)
+        assert list(ln) == [10, 8, 255, 0] and lit.tobytes() == blocks[1][1]
+
+
+def test_encoder_picks_raw_only_where_rans_does_not_pay():
+    rnd = W.generate("random", 4 * B, 7)
+    c, st = oracle.encode(rnd, return_stats=True, min_match=B)            # literals only
+    assert list(st.n_raw) == [4, 0, 0]                                   # every LIT stream raw, nothing else exists
+    # a raw literal-only block costs its bytes plus index entry, record header and padding
+    assert c.size - rnd.size <= 64 + 16 + 4 * (392 + 32 + 16) + 8 + 16
+    assert oracle.decode_all(c).tobytes() == rnd.tobytes()
+    c0, st0 = oracle.encode(rnd, return_stats=True, min_match=B, raw_slack_pct=0xFFFFFFFF)
+    assert list(st0.n_raw) == [0, 0, 0] and c0.size > c.size              # rANS on uniform bytes only adds its table
+    assert oracle.decode_all(c0).tobytes() == rnd.tobytes()
+    txt = W.generate("text", 4 * B, 7)
+    c1, st1 = oracle.encode(txt, return_stats=True, min_match=B)
+    assert st1.n_raw[0] == 0                                             # compressible literals stay entropy coded
+    # slack widens the margin monotonically and never changes the decoded bytes
+    fq = W.generate("fastq", 8 * B, 3)
+    prev = None
+    for pct in (0, 20, 1000):
+        c2, st2 = oracle.encode(fq, return_stats=True, raw_slack_pct=pct)
+        assert oracle.decode_all(c2).tobytes() == fq.tobytes()
+        n = sum(st2.n_raw)
+        assert prev is None or n >= prev
+        prev = n
+    assert prev == 3 * 8 - (8 - int(np.count_nonzero([oracle.decode_streams(c2, b)[0].n_seq for b in range(8)]))) * 2
+
+
+def test_rejects_inconsistent_raw_streams():
+    total, blocks = handmade_case()
+    recs = [build_record(b * B, s, l, raw=("len",)) for b, (s, l) in enumerate(blocks)]
+    good = build_container(total, recs)
+    assert oracle.decode_all(good).tobytes() == expand(total, blocks)
+    i = oracle.info(good)
+
+    def rejected(c):
+        with pytest.raises(oracle.OracleError):
+            oracle.decode_all(c)
+
+    bad = good.copy(); bad[i.payload_off + 7] = 0x08                      # reserved mode 2 for LEN
+    rejected(bad)
+    bad = good.copy(); bad[i.payload_off + 7] |= 0x40                     # reserved bits 6-7
+    rejected(bad)
+    bad = good.copy(); bad[i.payload_off + 8 + 4] ^= 1                    # n_words[LEN] != ceil(n_sym / 2)
+    rejected(bad)
+    bad = good.copy()
+    st = 64 + (i.n_blocks + 1) * 8 + (0 * 3 + 1) * 32 * 4 + 7 * 4         # block 0, LEN stream, lane 7
+    bad[st] ^= 1                                                          # an unused state that is not 2^16
+    rejected(bad)
+    # pad byte of an odd-length raw stream must be zero: block 2 has 1 sequence -> OFF stream of 2 bytes (even),
+    # so use a 3-byte literal stream
+    rec, stt = build_record(0, [], b"abc", raw=("lit",))
+    c = build_container(3, [(rec, stt)])
+    assert oracle.decode_all(c).tobytes() == b"abc"
+    pos = oracle.info(c).payload_off + 32 + 3                             # first section after the header = words[LIT]
+    bad = c.copy(); assert bad[pos] == 0; bad[pos] = 1
+    rejected(bad)
