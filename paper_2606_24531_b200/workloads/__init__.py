@@ -73,9 +73,10 @@ class Config:
 
 # Encoder policies. `literal` is the north_star wording taken literally (accept every match of
 # >= 4 bytes, no scheduling promises); `scheduled` is the policy the large configs run with
-# (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks.
+# (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks, in-block copy level 1,
+# and a stream is stored RAW when rANS would save less than 5 % of it (selective entropy).
 POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
-POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1)
+POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1, raw_slack_pct=5)
 
 CONFIGS = {
     "markov_1m": Config("markov_1m", "markov", 1 * MIB, SEED_BASE + 1, 4, POLICY_LITERAL,
