@@ -69,7 +69,8 @@ ScratchOffsets scratch_offsets(uint64_t n_blocks, const SlotLayout &sl, size_t n
     o.ctl = p; p += sizeof(Control);
     o.done = p; p += 4 * (size_t)n_blocks;
     o.mark = p; p += 4 * (size_t)n_blocks;
-    o.slot_of = p; p += 4 * (size_t)n_blocks;
+    p = align_up(p, 8);
+    o.slot_of = p; p += 8 * (size_t)n_blocks;
     o.zero_bytes = p;                          // everything up to here is zeroed by set_scratch
     p = align_up(p, 8);
     o.list = p; p += 8 * n_slots;
@@ -264,7 +265,7 @@ int aceapex_set_scratch(aceapex_ctx *c, void *d_scratch, size_t nbytes, size_t n
     c->sc.ctl = reinterpret_cast<Control *>(p + o.ctl);
     c->sc.done = reinterpret_cast<uint32_t *>(p + o.done);
     c->sc.mark = reinterpret_cast<uint32_t *>(p + o.mark);
-    c->sc.slot_of = reinterpret_cast<uint32_t *>(p + o.slot_of);
+    c->sc.slot_of = reinterpret_cast<unsigned long long *>(p + o.slot_of);
     c->sc.list = reinterpret_cast<uint64_t *>(p + o.list);
     c->sc.ids = reinterpret_cast<uint64_t *>(p + o.ids);
     c->sc.slots = p + o.slots;

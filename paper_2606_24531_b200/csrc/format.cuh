@@ -186,7 +186,7 @@ struct Scratch {
     Control *ctl;
     uint32_t *done;      // [n_blocks] epoch of the decode_all call that completed the block
     uint32_t *mark;      // [n_blocks] tag of the isolated-decode round that claimed the block
-    uint32_t *slot_of;   // [n_blocks] slot index assigned in that round
+    unsigned long long *slot_of;   // [n_blocks] round tag << 32 | slot index assigned in that round
     uint64_t *list;      // [n_slots]  block id held by each slot in this round
     uint64_t *ids;       // [n_targets] target block ids of the current group
     uint8_t *slots;      // n_slots * stride

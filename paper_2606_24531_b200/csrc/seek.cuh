@@ -122,7 +122,8 @@ __device__ inline void warp_parse_block(const Container &cv, const SlotLayout &s
 
 struct SeekArgs {
     uint64_t *pend;          // [nt][16384] per target byte: kDone | literal request | absolute position being chased
-    uint32_t *mark, *slot_of;
+    uint32_t *mark;          // [n_blocks] claim word: the tag of the round that claimed the block
+    unsigned long long *slot_of;   // [n_blocks] tag << 32 | slot, written by the claimer right after it won
     uint64_t *list;
     const uint64_t *ids;     // nt target ids (device); nullptr: the single target `one_id`
     uint64_t one_id;
@@ -138,18 +139,32 @@ constexpr unsigned long long kLitReq = 1ull << 62;   // pend = kLitReq | slot <<
 
 __device__ inline uint64_t seek_target(const SeekArgs &a, uint32_t i) { return a.ids ? a.ids[i] : a.one_id; }
 
-// Follow one byte through the parsed blocks that hold a slot in this round (mark == tag, slot index
-// below n_slots_ready) until it reaches a literal (-> literal request), leaves the resident set
-// (-> stays a position, claimed by the next hop's collect) or hits an inconsistency (-> kDone + status).
+// Claim a slot of round `tag` for block blk (once: the claim word decides the winner). The slot entry
+// carries the tag, so a reader can never pair a fresh claim with a stale slot index.
+__device__ inline void claim_block(const SeekArgs &a, Control *ctl, uint32_t tag, uint32_t rp, uint64_t blk)
+{
+    if (a.mark[blk] == tag) return;
+    if (atomicExch(a.mark + blk, tag) == tag) return;                  // somebody else claimed it
+    const uint32_t s = atomicAdd(&ctl->round_n_list[rp], 1u);
+    a.slot_of[blk] = (unsigned long long)tag << 32 | s;                // s >= max_slots: no slot in this round
+    if (s < a.max_slots) a.list[s] = blk;
+}
+
+// Follow one byte through the parsed blocks that hold a slot in this round (slot entry of this round's
+// tag with an index below n_ready, i.e. decoded and parsed before the last barrier) until it reaches a
+// literal (-> literal request), leaves the resident set (-> stays a position; its block is claimed on the
+// spot, for the next hop) or hits an inconsistency (-> kDone + status). Entries written during the
+// current phase have an index >= n_ready, and a stale cached entry can only carry an older tag: both
+// read as "not resident", which is always safe.
 __device__ inline unsigned long long chase_byte(const SlotLayout &sl, const SeekArgs &a, Control *ctl, uint32_t tag,
-                                                uint32_t n_ready, unsigned long long p)
+                                                uint32_t rp, uint32_t n_ready, unsigned long long p)
 {
     for (;;) {
         const uint64_t blk = p >> kBlockLog2;
         const uint32_t o = (uint32_t)(p & (kB - 1));
-        if (a.mark[blk] != tag) return p;
-        const uint32_t s = a.slot_of[blk];
-        if (s >= n_ready) return p;                                    // claimed, but no slot in this round
+        const unsigned long long e = a.slot_of[blk];
+        const uint32_t s = (uint32_t)e;
+        if ((uint32_t)(e >> 32) != tag || s >= n_ready) { claim_block(a, ctl, tag, rp, blk); return p; }
         uint8_t *slot = a.slots + (size_t)s * sl.stride;
         SlotHdr *h = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
         if (!h->parsed_ok) { raise(ctl, kStChase, blk); return kDone; }   // corrupt block: give up on this byte
@@ -224,26 +239,17 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv,
         const uint32_t rp = round & 1u, tag = a.tag0 + round;
         uint32_t n_ready = 0;                                          // slots of this round decoded and parsed
         unsigned long long chasing = 0;
+        // ---- round start: claim a slot for every distinct block a chasing byte sits in (later hops claim
+        //      on the spot, at the end of their chase)
+        for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
+            const uint64_t p = a.pend[g];
+            if (p < kLitReq) claim_block(a, ctl, tag, rp, p >> kBlockLog2);
+        }
+        grid_barrier(ctl, n_ctas);
         for (;; hop++) {
             const uint32_t hp = hop & 1u;
             SEEK_MARK(10);
-            // ---- collect: claim a slot for every distinct block a chasing byte sits in
-            for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
-                const uint64_t p = a.pend[g];
-                if (p >= kLitReq) continue;                            // done, or waiting for its literal
-                const uint64_t blk = p >> kBlockLog2;
-                if (a.mark[blk] == tag) continue;
-                if (atomicExch(a.mark + blk, tag) == tag) continue;    // somebody else claimed it
-                const uint32_t s = atomicAdd(&ctl->round_n_list[rp], 1u);
-                a.slot_of[blk] = s;                                    // s >= max_slots: no slot in this round
-                if (s < a.max_slots) a.list[s] = blk;
-            }
-            grid_barrier(ctl, n_ctas);
-            if (gtid == 0) {                                           // the other parities' counters are idle now
-                ctl->hop_pending[hp ^ 1u] = 0;
-                if (n_ready == 0) ctl->round_n_list[rp ^ 1u] = 0;
-            }
-            const uint32_t n_claimed = ctl->round_n_list[rp];
+            const uint32_t n_claimed = ld_acquire_u32(&ctl->round_n_list[rp]);
             const uint32_t n_now = n_claimed < a.max_slots ? n_claimed : a.max_slots;
             SEEK_MARK(11);
 #ifdef ACEAPEX_TRACE
@@ -257,6 +263,10 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv,
                 decode_unit(cv, sl, a.slots, a.list[bi], bi, so == 0 ? OFF : LEN, so == 1, ws, lane, ctl);
             }
             grid_barrier(ctl, n_ctas);
+            if (gtid == 0) {                                           // the other parities' counters are idle now
+                ctl->hop_pending[hp ^ 1u] = 0;
+                if (n_ready == 0) ctl->round_n_list[rp ^ 1u] = 0;
+            }
             SEEK_MARK(12);
             // ---- parse the new blocks, warp per block
             for (uint32_t bi = n_ready + gwarp; bi < n_now; bi += n_warps)
@@ -271,7 +281,7 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv,
             for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
                 const unsigned long long p = a.pend[g];
                 if (p >= kLitReq) continue;
-                const unsigned long long q = chase_byte(sl, a, ctl, tag, n_ready, p);
+                const unsigned long long q = chase_byte(sl, a, ctl, tag, rp, n_ready, p);
                 if (q != p) a.pend[g] = q;
                 remaining += q < kLitReq;
             }
@@ -282,6 +292,7 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv,
             grid_barrier(ctl, n_ctas);
             chasing = ctl->hop_pending[hp];
             SEEK_MARK(14);
+            // out of slots: the blocks claimed beyond max_slots wait for the next round
             if (chasing == 0 || n_claimed >= a.max_slots || hop + 1 >= a.max_hops) { hop++; break; }
         }
         // ---- literal phase: LIT stream of every slot with a request, then deliver
