@@ -154,6 +154,39 @@ __device__ inline Addr4 run_addresses(const uint2 *bm2, const uint16_t *rk, cons
     return a;
 }
 
+__device__ inline uint32_t ldg_u32(unsigned long long a)
+{
+    uint32_t v;
+    asm volatile("ld.global.u32 %0, [%1];" : "=r"(v) : "l"(a) : "memory");
+    return v;
+}
+
+// Word-granular plan of output bytes o .. o+3: the run of byte 0 (source address aA for byte 0), the
+// position k of the first run boundary inside the group (4 = none), the run of byte 3 (source address
+// aB for byte k) and whether there is a second boundary (then the group takes the per-byte path).
+// With at most one boundary the four bytes are k bytes at aA.. and 4-k bytes at aB..: two (unaligned)
+// 32-bit windows, each fetched as one or two ALIGNED words instead of four byte loads that touch the
+// same cache lines four times.
+#ifndef ACEAPEX_WORD_UNROLL
+#define ACEAPEX_WORD_UNROLL 4
+#endif
+constexpr uint32_t kWordUnroll = ACEAPEX_WORD_UNROLL;   // steps whose loads are in flight together
+struct GroupPlan { unsigned long long aA, aB; uint32_t k, multi; };
+__device__ inline GroupPlan plan_group(const uint2 *bm2, const uint16_t *rk, const unsigned long long *delta, uint32_t o)
+{
+    const uint2 w = bm2[o >> 5];
+    const uint32_t sh = o & 31u, m = (2u << sh) - 1u;
+    const uint32_t r0 = (uint32_t)rk[o >> 5] + __popc(w.x & m) + __popc(w.y & m);
+    const uint32_t t = (w.x >> sh) & 0xEu, u = (w.y >> sh) & 0xEu, x = t | u;
+    const uint32_t r3 = r0 + __popc(t) + __popc(u);                    // run of byte 3 (of byte k when there is one boundary)
+    GroupPlan g;
+    g.k = x ? (uint32_t)__ffs(x) - 1u : 4u;
+    g.multi = (x & (x - 1u)) != 0;
+    g.aA = delta[r0] + o;
+    g.aB = delta[r3] + o + (g.k & 3u);
+    return g;
+}
+
 __device__ inline void store4(unsigned long long a, uint32_t v, uint32_t aligned4)
 {
     if (aligned4) {
@@ -439,18 +472,50 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             // ---- pass 0: every output byte from delta[r(o)] + o; 16 byte loads in flight per thread
             const unsigned long long outB = (unsigned long long)__cvta_generic_to_global(out) + B0;
             uint32_t ob = 4 * tid;
-            for (; ob + 12 * kMatchThreads + 4 <= blen; ob += 16 * kMatchThreads) {
-                Addr4 a[4];
-                uint32_t b[4][4];
+            if (out_aligned4) {
+                // word-granular gather (see plan_group): per step up to 4 aligned word loads, predicated on need
+                for (; ob + (kWordUnroll - 1) * 4 * kMatchThreads + 4 <= blen; ob += kWordUnroll * 4 * kMatchThreads) {
+                    GroupPlan g[kWordUnroll];
+                    uint32_t alo[kWordUnroll], ahi[kWordUnroll], blo[kWordUnroll], bhi[kWordUnroll], v[kWordUnroll];
 #pragma unroll
-                for (int u = 0; u < 4; u++) a[u] = run_addresses(bm2, rk, delta, ob + u * 4 * kMatchThreads);
+                    for (int u = 0; u < (int)kWordUnroll; u++) g[u] = plan_group(bm2, rk, delta, ob + u * 4 * kMatchThreads);
 #pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    b[u][0] = ldg_u8(a[u].a0); b[u][1] = ldg_u8(a[u].a1); b[u][2] = ldg_u8(a[u].a2); b[u][3] = ldg_u8(a[u].a3);
+                    for (int u = 0; u < (int)kWordUnroll; u++) {
+                        const unsigned long long wa = g[u].aA & ~3ull, wb = g[u].aB & ~3ull;
+                        const uint32_t fa = (uint32_t)g[u].aA & 3u, fb = (uint32_t)g[u].aB & 3u, k = g[u].k;
+                        alo[u] = ldg_u32(wa);
+                        ahi[u] = fa + k > 4 ? ldg_u32(wa + 4) : 0u;            // k = 4 for a group inside one run
+                        blo[u] = k < 4 ? ldg_u32(wb) : 0u;
+                        bhi[u] = (k < 4 && fb + (4 - k) > 4) ? ldg_u32(wb + 4) : 0u;
+                    }
+#pragma unroll
+                    for (int u = 0; u < (int)kWordUnroll; u++) {
+                        const uint32_t k = g[u].k;
+                        const uint32_t va = __funnelshift_r(alo[u], ahi[u], 8 * ((uint32_t)g[u].aA & 3u));
+                        const uint32_t vb = __funnelshift_r(blo[u], bhi[u], 8 * ((uint32_t)g[u].aB & 3u));
+                        v[u] = k < 4 ? (va & ((1u << (8 * k)) - 1u)) | (vb << (8 * k)) : va;
+                        if (g[u].multi) {                                      // two or more boundaries: byte by byte
+                            const Addr4 a = run_addresses(bm2, rk, delta, ob + u * 4 * kMatchThreads);
+                            v[u] = ldg_u8(a.a0) | ldg_u8(a.a1) << 8 | ldg_u8(a.a2) << 16 | ldg_u8(a.a3) << 24;
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < (int)kWordUnroll; u++) store4(outB + ob + u * 4 * kMatchThreads, v[u], 1u);
                 }
+            } else {
+                for (; ob + 12 * kMatchThreads + 4 <= blen; ob += 16 * kMatchThreads) {
+                    Addr4 a[4];
+                    uint32_t b[4][4];
 #pragma unroll
-                for (int u = 0; u < 4; u++)
-                    store4(outB + ob + u * 4 * kMatchThreads, b[u][0] | b[u][1] << 8 | b[u][2] << 16 | b[u][3] << 24, out_aligned4);
+                    for (int u = 0; u < 4; u++) a[u] = run_addresses(bm2, rk, delta, ob + u * 4 * kMatchThreads);
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        b[u][0] = ldg_u8(a[u].a0); b[u][1] = ldg_u8(a[u].a1); b[u][2] = ldg_u8(a[u].a2); b[u][3] = ldg_u8(a[u].a3);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; u++)
+                        store4(outB + ob + u * 4 * kMatchThreads, b[u][0] | b[u][1] << 8 | b[u][2] << 16 | b[u][3] << 24, 0u);
+                }
             }
             for (; ob + 4 <= blen; ob += 4 * kMatchThreads) {
                 const Addr4 a = run_addresses(bm2, rk, delta, ob);
