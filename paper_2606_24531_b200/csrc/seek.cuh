@@ -40,65 +40,106 @@ __device__ inline void grid_barrier(Control *ctl, uint32_t n_ctas)
     __syncthreads();
 }
 
-// Parse the decoded LEN / OFF streams of the block in `slot` into the slot's token arrays, by ONE warp
-// (FORMAT.md section 4; same rules as the match kernel's parse, restated for a warp: 32 sequences per
-// round, one packed warp scan, carries in registers). Sets hdr->parsed_ok.
-__device__ inline void warp_parse_block(const Container &cv, const SlotLayout &sl, uint8_t *slot, uint64_t blk,
-                                        Control *ctl, uint32_t lane)
+// Parse the decoded LEN / OFF streams of the block in `slot` into the slot's token arrays (FORMAT.md
+// section 4; same rules as the match kernel's parse). FOUR warps share a block, each a contiguous
+// quarter of its sequences (the phase is pure latency, so the rounds are spread): pass 0 counts the
+// length escapes of each quarter, pass 1 sums the lengths, pass 2 - with the quarter's bases known -
+// scans and writes start / dst / litpos / src and checks every match. The passes are separated by CTA
+// barriers: all warps of the CTA call this the same number of times (idle quads pass slot == nullptr).
+//   sq: shared exchange area of the quad, uint32_t [4][4].
+__device__ inline void quad_parse_block(const Container &cv, const SlotLayout &sl, uint8_t *slot, uint64_t blk,
+                                        Control *ctl, uint32_t lane, uint32_t r /* warp in quad */, uint32_t (*sq)[4])
 {
-    SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
-    bool ok = !(hdr->bad[LEN] | hdr->bad[OFF]);                        // the LIT stream is decoded later, on demand
-    const uint32_t n = hdr->n_seq, n_lit = hdr->n_lit, blen = hdr->block_len, n_extras = hdr->n_extras;
-    const uint32_t onb = hdr->off_nbytes;
-    ok = ok && n <= sl.ms && onb >= 1 && onb <= 8;
+    SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot ? slot + sl.o_hdr : nullptr);
+    bool ok = slot != nullptr;
+    uint32_t n = 0, n_lit = 0, blen = 0, n_extras = 0, onb = 1;
     if (ok) {
-        const uint16_t *len16 = reinterpret_cast<const uint16_t *>(slot + sl.o_len);
-        const uint8_t *off_s = slot + sl.o_off;
-        const uint16_t *extras = reinterpret_cast<const uint16_t *>(cv.payload + ((uint64_t)hdr->rec_lo | (uint64_t)hdr->rec_hi << 32) +
-                                                                    hdr->extras_off);
+        ok = !(hdr->bad[LEN] | hdr->bad[OFF]);                         // the LIT stream is decoded later, on demand
+        n = hdr->n_seq; n_lit = hdr->n_lit; blen = hdr->block_len; n_extras = hdr->n_extras; onb = hdr->off_nbytes;
+        ok = ok && n <= sl.ms && onb >= 1 && onb <= 8;
+    }
+    if (!ok) n = 0;
+    const uint32_t cq = ((n + 127) / 128) * 32;                        // sequences per warp, a multiple of 32
+    const uint32_t k0 = min(n, r * cq), k1 = min(n, k0 + cq);
+    const uint16_t *len16 = reinterpret_cast<const uint16_t *>(slot ? slot + sl.o_len : nullptr);
+    const uint8_t *off_s = slot ? slot + sl.o_off : nullptr;
+    const uint16_t *extras = ok ? reinterpret_cast<const uint16_t *>(cv.payload + ((uint64_t)hdr->rec_lo | (uint64_t)hdr->rec_hi << 32) +
+                                                                     hdr->extras_off) : nullptr;
+    // ---- pass 0: escapes per quarter
+    uint32_t esc = 0;
+    for (uint32_t k = k0 + lane; k < k1; k += 32) { const uint32_t v = len16[k]; esc += ((v & 0xFFu) == 255) + ((v >> 8) == 255); }
+    esc = __reduce_add_sync(0xFFFFFFFFu, esc);
+    if (lane == 0) sq[r][0] = esc;
+    __syncthreads();
+    uint32_t e0 = 0, e_all = 0;
+    for (uint32_t i = 0; i < 4; i++) { const uint32_t x = sq[i][0]; if (i < r) e0 += x; e_all += x; }
+    bool bad = e_all != n_extras;                                      // quad-uniform; bounds every extras index below
+    // ---- pass 1: length sums per quarter (true values through the escapes)
+    uint32_t s_ll = 0, s_all = 0;
+    if (!bad) {
+        uint32_t e = e0;
+        for (uint32_t kb = k0; kb < k1; kb += 32) {
+            const uint32_t k = kb + lane;
+            uint32_t ll = 0, ml = 0;
+            if (k < k1) { const uint32_t v = len16[k]; ll = v & 0xFFu; ml = (v >> 8) + 4; }
+            if (n_extras) {
+                const uint32_t e_ll = ll == 255, e_ml = ml == 259;
+                uint32_t etot;
+                uint32_t ei = e + warp_excl_scan(e_ll + e_ml, lane, etot);
+                e += etot;
+                if (e_ll) ll = extras[ei++];
+                if (e_ml) ml = (uint32_t)extras[ei] + 4;
+            }
+            s_ll += ll; s_all += ll + ml;
+        }
+        s_ll = __reduce_add_sync(0xFFFFFFFFu, s_ll);
+        s_all = __reduce_add_sync(0xFFFFFFFFu, s_all);
+    }
+    if (lane == 0) { sq[r][1] = s_ll; sq[r][2] = s_all; }
+    __syncthreads();
+    uint32_t lp = 0, pos = 0, t_ll = 0, t_all = 0;
+    for (uint32_t i = 0; i < 4; i++) { const uint32_t x = sq[i][1], y = sq[i][2]; if (i < r) { lp += x; pos += y; } t_ll += x; t_all += y; }
+    if (!bad) bad = t_ll > n_lit || t_all + (n_lit - t_ll) != blen;    // quad-uniform; every position below is < 16384
+    // ---- pass 2: scan, token arrays, per-match checks
+    if (!bad && ok) {
         uint16_t *start = reinterpret_cast<uint16_t *>(slot + sl.o_start);
         uint16_t *dst = reinterpret_cast<uint16_t *>(slot + sl.o_dst);
         uint16_t *litpos = reinterpret_cast<uint16_t *>(slot + sl.o_litpos);
         uint64_t *srcv = reinterpret_cast<uint64_t *>(slot + sl.o_src);
         const uint64_t B0 = blk << kBlockLog2;
-        uint32_t lp = 0, pos = 0, e = 0;                               // warp-uniform carries
-        bool bad = false;
         const uint64_t src_mask = ~0ull >> (64 - 8 * onb);
-        // loads of round i+1 are issued before round i is processed (one warp: latency is everything)
+        uint32_t e = e0;
+        // loads of round i+1 are issued before round i is processed
         uint32_t v_nx = 0, w0_nx = 0, w1_nx = 0, w2_nx = 0;
         auto fetch = [&](uint32_t k) {
             v_nx = w0_nx = w1_nx = w2_nx = 0;
-            if (k < n) {
+            if (k < k1) {
                 v_nx = len16[k];
                 const uint32_t *wp = reinterpret_cast<const uint32_t *>(off_s + ((k * onb) & ~3u));   // stays inside the slot
                 w0_nx = wp[0]; w1_nx = wp[1]; w2_nx = wp[2];
             }
         };
-        fetch(lane);
-        for (uint32_t kb = 0; kb < n; kb += 32) {
+        fetch(k0 + lane);
+        bool mbad = false;
+        for (uint32_t kb = k0; kb < k1; kb += 32) {
             const uint32_t k = kb + lane;
-            const bool act = k < n;
+            const bool act = k < k1;
             const uint32_t v = v_nx, w0 = w0_nx, w1 = w1_nx, w2 = w2_nx;
             fetch(k + 32);
             uint32_t ll = 0, ml = 0;
             if (act) { ll = v & 0xFFu; ml = (v >> 8) + 4; }
-            if (n_extras) {                                            // warp-uniform: escapes are rare
+            if (n_extras) {
                 const uint32_t e_ll = ll == 255, e_ml = ml == 259;
                 uint32_t etot;
                 uint32_t ei = e + warp_excl_scan(e_ll + e_ml, lane, etot);
                 e += etot;
-                if (e > n_extras) { bad = true; break; }               // warp-uniform
                 if (e_ll) ll = extras[ei++];
                 if (e_ml) ml = (uint32_t)extras[ei] + 4;
-            } else if (ll == 255 || ml == 259) {
-                bad = true;                                            // an escape without extras
             }
-            // an invalid stream may overflow 16 bits, so the two running sums are scanned apart
-            uint32_t t_ll, t_all;
-            const uint32_t p_ll = warp_excl_scan(ll, lane, t_ll), p_all = warp_excl_scan(ll + ml, lane, t_all);
-            const uint32_t my_lp = lp + p_ll, my_st = pos + p_all;
-            lp += t_ll; pos += t_all;
-            if (lp > n_lit || pos > blen) { bad = true; break; }       // warp-uniform; bounds every value below
+            uint32_t ptot;
+            const uint32_t pre = warp_excl_scan(ll | (ll + ml) << 16, lane, ptot);   // sums validated: no overflow
+            const uint32_t my_lp = lp + (pre & 0xFFFFu), my_st = pos + (pre >> 16);
+            lp += ptot & 0xFFFFu; pos += ptot >> 16;
             if (act) {
                 const uint32_t sh = ((k * onb) & 3u) * 8;
                 const uint32_t lo = __funnelshift_r(w0, w1, sh), hi = __funnelshift_r(w1, w2, sh);
@@ -107,17 +148,20 @@ __device__ inline void warp_parse_block(const Container &cv, const SlotLayout &s
                 litpos[k] = (uint16_t)my_lp;
                 dst[k] = (uint16_t)(my_st + ll);
                 srcv[k] = src;
-                if (src + ml > B0 + my_st + ll) bad = true;            // strictly before, non-overlapping
+                if (src + ml > B0 + my_st + ll) mbad = true;           // strictly before, non-overlapping
             }
         }
-        bad = __any_sync(0xFFFFFFFFu, bad);
-        if (!bad) bad = e != n_extras || pos + (n_lit - lp) != blen;
-        if (!bad && lane == 0) { start[n] = (uint16_t)pos; litpos[n] = (uint16_t)lp; }
-        ok = !bad;
-        if (!ok && lane == 0) raise(ctl, kStTokens, blk);
+        if (__any_sync(0xFFFFFFFFu, mbad)) bad = true;
+        if (r == 3 && lane == 0) { start[n] = (uint16_t)t_all; litpos[n] = (uint16_t)t_ll; }
     }
-    if (lane == 0) hdr->parsed_ok = ok ? 1u : 0u;
-    __syncwarp();
+    if (lane == 0) sq[r][3] = bad ? 1u : 0u;
+    __syncthreads();
+    if (slot && r == 0 && lane == 0) {
+        const bool good = ok && !(sq[0][3] | sq[1][3] | sq[2][3] | sq[3][3]);
+        if (ok && !good) raise(ctl, kStTokens, blk);
+        hdr->parsed_ok = good ? 1u : 0u;
+    }
+    __syncthreads();                                                   // sq is reused by the next call
 }
 
 struct SeekArgs {
@@ -198,10 +242,11 @@ __device__ inline unsigned long long chase_byte(const SlotLayout &sl, const Seek
 //   until nothing is chasing (or the slots are used up); then ONE literal phase:
 //   entropy-decode the LIT stream of the slots that received a literal request, deliver the bytes.
 // A seek therefore pays for the long LIT streams once, not once per hop, and ends on the device.
-__global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv, SlotLayout sl, SeekArgs a, Control *ctl)
+__global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container cv, SlotLayout sl, SeekArgs a, Control *ctl)
 {
     extern __shared__ __align__(1024) uint8_t smem_entropy[];
     __shared__ uint32_t s_rem;
+    __shared__ uint32_t s_quad[kEntropyWarps / 4][4][4];
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
     WarpSmem ws;
     {
@@ -268,9 +313,12 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_seek_fused(Container cv,
                 if (n_ready == 0) ctl->round_n_list[rp ^ 1u] = 0;
             }
             SEEK_MARK(12);
-            // ---- parse the new blocks, warp per block
-            for (uint32_t bi = n_ready + gwarp; bi < n_now; bi += n_warps)
-                warp_parse_block(cv, sl, a.slots + (size_t)bi * sl.stride, a.list[bi], ctl, lane);
+            // ---- parse the new blocks, four warps per block
+            for (uint32_t b0 = n_ready + blockIdx.x * (kEntropyWarps / 4); b0 < n_now; b0 += n_ctas * (kEntropyWarps / 4)) {
+                const uint32_t bi = b0 + (warp >> 2);
+                uint8_t *slot = bi < n_now ? a.slots + (size_t)bi * sl.stride : nullptr;
+                quad_parse_block(cv, sl, slot, slot ? a.list[bi] : 0, ctl, lane, warp & 3u, s_quad[warp >> 2]);
+            }
             grid_barrier(ctl, n_ctas);
             SEEK_MARK(13);
             n_ready = n_now;
