@@ -107,7 +107,7 @@ uint32_t match_grid(aceapex_ctx *c, uint32_t count)
 }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
-                   uint32_t count, cudaStream_t st)
+                   uint32_t count, cudaStream_t st, uint32_t reset_watermark = 0)
 {
     uint32_t units = 3 * (list ? max_slots : count);
     uint32_t grid = (units + kEntropyWarps - 1) / kEntropyWarps;
@@ -117,7 +117,7 @@ int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list,
     {
         LaunchScope ls(c, K_ENTROPY, st);
         k_entropy<<<grid, 32 * kEntropyWarps, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
-                                                     c->sc.ctl);
+                                                     c->sc.ctl, reset_watermark);
     }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
 }
@@ -291,12 +291,12 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         if (cudaMemsetAsync(c->sc.done, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
         c->epoch = 1;
     }
-    if (cudaMemsetAsync(&c->sc.ctl->watermark, 0, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
     const uint32_t aligned = ((uintptr_t)d_out & 3) == 0;
     for (uint64_t first = 0; first < c->cv.n_blocks; first += c->sc.n_slots) {
         const uint64_t rest = c->cv.n_blocks - first;
         const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);
-        int rc = launch_entropy(c, nullptr, nullptr, 0, first, count, st);
+        // the first entropy launch of the call also resets the watermark (nothing reads it before the match kernel)
+        int rc = launch_entropy(c, nullptr, nullptr, 0, first, count, st, first == 0 ? 1u : 0u);
         if (rc != ACEAPEX_OK) return rc;
         {
             LaunchScope ls(c, K_MATCH, st);

@@ -308,10 +308,11 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
 // Unit u -> stream u / nb in the order LIT, OFF, LEN; block index u % nb (= slot). Output: the slot's areas.
 __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, SlotLayout sl, uint8_t *slots, const uint64_t *list,
                                                  const uint32_t *n_list, uint32_t max_slots, uint64_t first,
-                                                 uint32_t count, Control *ctl)
+                                                 uint32_t count, Control *ctl, uint32_t reset_watermark)
 {
     extern __shared__ __align__(1024) uint8_t smem_entropy[];
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    if (reset_watermark && blockIdx.x == 0 && threadIdx.x == 0) ctl->watermark = 0;   // decode_all: first launch of a call
     WarpSmem ws;
     {
         const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(smem_entropy);
