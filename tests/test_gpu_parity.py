@@ -115,6 +115,28 @@ def test_bench_config_fastq_64m_full_size(binding):
     full_check(binding, c, want, seek_blocks=ids, n_targets=64)
 
 
+@pytest.mark.parametrize("name", ["genome_256m", "text_256m"])
+def test_configs_2_3_full_size(binding, name):
+    """BASELINE.json configs[2] (8-byte offsets) and configs[3] at full size (16,384 blocks): decode_all against
+    the original bytes (round-trip identity pins the oracle), sampled isolated blocks against oracle decoder #2."""
+    cfg = W.CONFIGS[name]
+    data = cfg.data()
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=8, **cfg.encoder)
+    assert oracle.info(c).offset_width == cfg.offset_width
+    nb = int(oracle.info(c).n_blocks)
+    ids = [int(x) for x in W.seek_ids(nb, 24, W.SEED_BASE + 0x73)] + [0, nb - 1]
+    with binding.Decoder(c, n_targets=32) as dec, oracle.Isolated(c) as iso:
+        out = dev_out(data.size)
+        dec.decode_all(out)
+        dec.check()
+        assert torch.equal(out.cpu(), torch.from_numpy(data))
+        got = dec.decode_blocks(np.array(ids, np.uint64), dev_out(len(ids) * B)).cpu().numpy()
+        dec.check()
+        for i, b in enumerate(ids):
+            blk = iso.decode(b)
+            assert np.array_equal(got[i * B:i * B + blk.size], blk), b
+
+
 # ------------------------------------------------------------------ entropy layer alone
 
 @pytest.mark.parametrize("name", ["markov_1m", "genome_256m"])
