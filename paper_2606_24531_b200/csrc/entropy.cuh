@@ -255,7 +255,12 @@ __device__ inline bool copy_raw_stream(uint32_t x, uint32_t n, const uint8_t *wo
     const uint4 *src = reinterpret_cast<const uint4 *>(words_sec);
     uint4 *dst = reinterpret_cast<uint4 *>(out);
     const uint32_t nv = (n + 15) >> 4;
-    for (uint32_t i = lane; i < nv; i += 32) dst[i] = src[i];
+    uint32_t i = lane;
+    for (; i + 96 < nv; i += 128) {                                    // four loads in flight per lane
+        const uint4 a = src[i], b = src[i + 32], c = src[i + 64], d = src[i + 96];
+        dst[i] = a; dst[i + 32] = b; dst[i + 64] = c; dst[i + 96] = d;
+    }
+    for (; i < nv; i += 32) dst[i] = src[i];
     if ((n & 1u) && lane == 0 && words_sec[n] != 0) ok = false;
     return __all_sync(0xFFFFFFFFu, ok);
 }
