@@ -472,7 +472,16 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             // ---- pass 0: every output byte from delta[r(o)] + o; 16 byte loads in flight per thread
             const unsigned long long outB = (unsigned long long)__cvta_generic_to_global(out) + B0;
             uint32_t ob = 4 * tid;
-            if (out_aligned4) {
+            if (n == 0 && out_aligned4) {
+                // a block without matches (incompressible data) is its literal stream: straight word copy
+                const uint32_t *lw = reinterpret_cast<const uint32_t *>(slot + sl.o_lit);
+                for (; ob + 12 * kMatchThreads + 4 <= blen; ob += 16 * kMatchThreads) {
+                    const uint32_t i = ob >> 2;
+                    const uint32_t a = lw[i], b = lw[i + kMatchThreads], c = lw[i + 2 * kMatchThreads], d = lw[i + 3 * kMatchThreads];
+                    store4(outB + ob, a, 1u); store4(outB + ob + 4 * kMatchThreads, b, 1u);
+                    store4(outB + ob + 8 * kMatchThreads, c, 1u); store4(outB + ob + 12 * kMatchThreads, d, 1u);
+                }
+            } else if (out_aligned4) {
                 // word-granular gather (see plan_group): per step up to 4 aligned word loads, predicated on need
                 for (; ob + (kWordUnroll - 1) * 4 * kMatchThreads + 4 <= blen; ob += kWordUnroll * 4 * kMatchThreads) {
                     GroupPlan g[kWordUnroll];
