@@ -119,17 +119,16 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
 struct Control {
     unsigned long long first_bad;   // lowest block id that raised a status bit (atomicMin)
     unsigned long long watermark;   // decode_all: number of leading blocks complete
-    unsigned long long pending;     // isolated decode: bytes still unresolved after a hop
+    unsigned long long rsv0;
     uint32_t status;                // sticky kSt* bits
     uint32_t ticket, ticket_exit;   // decode_all match kernel: ordered block hand-out
     uint32_t unit, unit_exit;       // entropy kernel: (block, stream) unit hand-out
-    uint32_t n_list;                // (unused since the fused isolated kernel; kept for layout)
+    uint32_t rsv1;
     uint32_t max_n_seq;             // open-time scan result
-    // fused isolated decode (seek.cuh): grid barrier and per-hop counters, double-buffered by hop parity
+    // fused isolated decode (seek.cuh): grid barrier and counters, double-buffered by round / hop parity
     uint32_t bar_count, bar_gen;
     uint32_t round_n_list[2];       // distinct blocks claimed so far in the round (by round parity)
-    uint32_t hop_unit[2];           // (unused)
-    uint32_t pad0;
+    uint32_t rsv2[3];
     unsigned long long hop_pending[2];   // bytes still chasing after the hop (by hop parity)
     uint32_t pad[8];
 };

@@ -31,17 +31,15 @@ __device__ inline void st_release_u32(uint32_t *p, uint32_t v)
 // Cross-block ordering. A finished block publishes its done flag (epoch of this call) with release
 // semantics; the flag store follows the CTA barrier that ends the block's writes, and a release is
 // cumulative over what the barrier ordered before it, so one thread publishes for the whole CTA.
-// The watermark (number of leading complete blocks) is advanced lazily by whoever needs it: a CTA
-// whose block copies from earlier blocks scans the done flags from the watermark on, 32 per round
-// trip with acquire loads, until everything below its highest source block is complete, and leaves
-// the new watermark behind for the next one (atomicMax after a fence, so that a later reader of the
-// watermark also sees those blocks' bytes). Block ids are handed out in increasing order, so every
-// block a CTA waits for belongs to a CTA that is running or finished: no deadlock.
-//
-// When the header promises a window R, a block knows before it has parsed anything that its sources
-// end below block blk - R + 1: one warp runs the scan up to there while the block's streams are still
-// in flight (blocking = false: it stops at the first incomplete block instead of spinning), and the
-// blocking call after the parse usually finds nothing left to do.
+// The watermark (number of leading complete blocks) is kept moving by a helper CTA (ticket 0 of the
+// match kernel), which scans the done flags with acquire loads and publishes the new value with a
+// fence + atomicMax, so that whoever later acquires the watermark also sees those blocks' bytes.
+// A block reads the watermark once, early; if that value does not cover its highest source block yet
+// (no window promise, or the helper lags), its first warp scans the flags itself with the function
+// below - correct for any valid stream, with or without the helper. Block ids are handed out in
+// increasing order, so every block a CTA waits for belongs to a CTA that is running or finished: no
+// deadlock.
+//   blocking = false stops at the first incomplete block instead of spinning (the helper's mode).
 __device__ inline unsigned long long wait_for_blocks(Control *ctl, const uint32_t *done, uint32_t epoch,
                                                      unsigned long long w, unsigned long long below, bool blocking)
 {
