@@ -404,3 +404,24 @@ def test_rejects_inconsistent_raw_streams(binding):
     full_check(binding, c, np.frombuffer(b"abc", np.uint8), n_targets=1)
     bad = c.copy(); bad[oracle.info(c).payload_off + 32 + 3] = 1          # pad byte of the odd raw stream
     expect_corrupt(binding, bad, 3, 0)
+
+
+# ------------------------------------------------------------------ seeded fuzz over sizes and encoder policies
+
+def test_fuzz_small_containers(binding):
+    """40 seeded combinations of profile, size (ragged tails included), offset width, match threshold, depth
+    bound, window, in-block level cap and RAW slack; decode_all and every block in isolation, few slots."""
+    rng = np.random.default_rng(0xACEA9E)
+    kinds = ["markov", "fastq", "genome", "text", "random", "mixed"]
+    for it in range(40):
+        kind = kinds[it % len(kinds)]
+        n = int(rng.integers(1, 14 * B))
+        data = W.generate(kind, n, 1000 + it)
+        window = int(rng.choice([0, 0, 1, 2, 5]))
+        params = dict(min_match=int(rng.choice([4, 5, 8, 16])), max_depth=int(rng.choice([0, 1, 3, 8])), window=window,
+                      batch=int(rng.choice([1, 2, 4])) if window else 64, max_level=int(rng.choice([1, 2, 15])),
+                      raw_slack_pct=int(rng.choice([0, 0, 25, 1000, 0xFFFFFFFF])), offset_width=int(rng.choice([4, 8])))
+        c = oracle.encode(data, **params)
+        want = oracle.decode_all(c)
+        assert np.array_equal(want, data), (it, kind, n, params)
+        full_check(binding, c, want, n_slots=int(rng.choice([1, 3, 64])), n_targets=int(rng.choice([1, 2, 16])))
