@@ -409,11 +409,11 @@ def test_rejects_inconsistent_raw_streams(binding):
 # ------------------------------------------------------------------ seeded fuzz over sizes and encoder policies
 
 def test_fuzz_small_containers(binding):
-    """40 seeded combinations of profile, size (ragged tails included), offset width, match threshold, depth
+    """120 seeded combinations of profile, size (ragged tails included), offset width, match threshold, depth
     bound, window, in-block level cap and RAW slack; decode_all and every block in isolation, few slots."""
     rng = np.random.default_rng(0xACEA9E)
     kinds = ["markov", "fastq", "genome", "text", "random", "mixed"]
-    for it in range(40):
+    for it in range(120):
         kind = kinds[it % len(kinds)]
         n = int(rng.integers(1, 14 * B))
         data = W.generate(kind, n, 1000 + it)
@@ -425,3 +425,38 @@ def test_fuzz_small_containers(binding):
         want = oracle.decode_all(c)
         assert np.array_equal(want, data), (it, kind, n, params)
         full_check(binding, c, want, n_slots=int(rng.choice([1, 3, 64])), n_targets=int(rng.choice([1, 2, 16])))
+
+
+def test_fuzz_corrupted_containers_never_escape_their_buffers(binding):
+    """100 seeded containers with 1-3 flipped bytes anywhere behind the container header: open either rejects
+    them or decode_all / decode_blocks run to completion, never write beyond total_len (resp. the listed blocks)
+    and report either OK or CORRUPT (a flip inside literal or offset data is not detectable without a checksum)."""
+    rng = np.random.default_rng(7)
+    seen = {"rejected": 0, "ok": 0, "corrupt": 0}
+    for it in range(100):
+        kind = ["fastq", "text", "genome", "mixed"][it % 4]
+        n = int(rng.integers(2 * B, 9 * B))
+        data = W.generate(kind, n, 500 + it)
+        c = oracle.encode(data, min_match=8, max_depth=8, window=int(rng.choice([0, 2])), batch=2,
+                          raw_slack_pct=int(rng.choice([0, 1000])))
+        bad = c.copy()
+        for _ in range(int(rng.integers(1, 4))):
+            bad[int(rng.integers(64, bad.size))] ^= int(rng.integers(1, 256))
+        try:
+            dec = binding.Decoder(bad, n_targets=2, n_slots=int(rng.choice([2, 64])))
+        except binding.AceapexError:
+            seen["rejected"] += 1
+            continue
+        with dec:
+            out = dev_out(n + 4096)
+            dec.decode_all(out)
+            rc, _ = dec.device_status(clear=True)
+            assert rc in (0, binding.E_CORRUPT)
+            assert np.all(out.cpu().numpy()[n:] == 0xA5)
+            seen["ok" if rc == 0 else "corrupt"] += 1
+            ids = np.array([int(rng.integers(0, (n + B - 1) // B)) for _ in range(2)], np.uint64)
+            buf = dev_out(2 * B + 64)
+            dec.decode_blocks(ids, buf)
+            assert dec.device_status(clear=True)[0] in (0, binding.E_CORRUPT)
+            assert np.all(buf.cpu().numpy()[2 * B:] == 0xA5)
+    assert seen["corrupt"] >= 40                                     # most flips land in entropy-coded data
