@@ -113,7 +113,7 @@ class Decoder:
         self.info = Info()
         _check(L.aceapex_info_get(self._ctx, C.byref(self.info)), "aceapex_info_get")
         self.scratch = None
-        self.set_scratch(n_slots if n_slots is not None else max(1, min(int(self.info.n_blocks), 16384)), n_targets)
+        self.set_scratch(n_slots if n_slots is not None else max(1, min(int(self.info.n_blocks), 65536)), n_targets)
 
     # -- aceapex_scratch_bytes / aceapex_set_scratch
     def set_scratch(self, n_slots: int, n_targets: int, stream=None):
