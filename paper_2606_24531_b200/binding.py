@@ -91,7 +91,7 @@ def _stream_ptr(stream) -> int:
 class Decoder:
     """One opened container resident in device memory (``aceapex_open`` .. ``aceapex_close``)."""
 
-    def __init__(self, container, n_slots: int | None = None, n_targets: int = 64, device="cuda:0"):
+    def __init__(self, container, n_slots: int | None = None, n_targets: int = 256, device="cuda:0"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_24531_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
