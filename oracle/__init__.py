@@ -93,6 +93,7 @@ def lib():
             L.ora_decode_streams.argtypes = [u8p, sz, C.c_uint64, C.POINTER(BlockHdr), vp, vp, vp, vp, vp]
             L.ora_decode_tokens.argtypes = [u8p, sz, C.c_uint64, C.POINTER(C.c_uint32), vp, vp, vp, vp]
             L.ora_decode_all.argtypes = [u8p, sz, u8p, sz]
+            L.ora_decode_all_mt.argtypes = [u8p, sz, u8p, sz, C.c_uint32]
             L.ora_iso_open.argtypes = [u8p, sz, C.POINTER(vp)]
             L.ora_iso_decode.argtypes = [vp, C.c_uint64, u8p, sz, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
             L.ora_iso_close.argtypes = [vp]; L.ora_iso_close.restype = None
@@ -190,6 +191,15 @@ def decode_all(container) -> np.ndarray:
     i = info(c)
     out = np.full(max(1, i.total_len), 0xA5, dtype=np.uint8)
     _check(lib().ora_decode_all(_ptr(c), c.size, _ptr(out), i.total_len), "decode_all")
+    return out[: i.total_len]
+
+
+def decode_all_mt(container, threads: int) -> np.ndarray:
+    """Decoder #1 with the entropy stage on `threads` host threads, the match stage in block order."""
+    c = _bytes_arr(container)
+    i = info(c)
+    out = np.full(max(1, i.total_len), 0xA5, dtype=np.uint8)
+    _check(lib().ora_decode_all_mt(_ptr(c), c.size, _ptr(out), i.total_len, threads), "decode_all_mt")
     return out[: i.total_len]
 
 

@@ -115,6 +115,11 @@ int ora_decode_tokens(const uint8_t *c, size_t clen, uint64_t block, uint32_t *n
 /* Decoder #1: sequential, block order (defines decode_all). Writes out[0,total_len). */
 int ora_decode_all(const uint8_t *c, size_t clen, uint8_t *out, size_t cap);
 
+/* The same decoder with the entropy stage (steps 2.1-2.3, independent per block) spread over
+ * `threads` host threads and the match stage (step 2.4) in block order on one thread; the multi-core CPU
+ * baseline of SURVEY.md section 8(d). Bit-identical to ora_decode_all. */
+int ora_decode_all_mt(const uint8_t *c, size_t clen, uint8_t *out, size_t cap, uint32_t threads);
+
 /* Decoder #2: per-byte origin chase (defines seek / decode_blocks). Independent algorithm.
  * Writes only dst[0, block_len). The context memoises parsed blocks. */
 typedef struct ora_iso ora_iso;

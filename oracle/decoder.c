@@ -233,6 +233,25 @@ int ora_decode_tokens(const uint8_t *c, size_t clen, uint64_t block, uint32_t *n
 
 /* ---------------------------------------------------------------- decoder #1 */
 
+/* decoder #1 step 2.4: emit one block from its tokens (literal run, then memcpy from the absolute position) */
+static int emit_block(const ora_tokens *t, uint64_t b, uint8_t *out)
+{
+    uint64_t pos = b * ORA_B, end = pos + t->block_len;
+    uint32_t lp = 0;
+    for (uint32_t q = 0; q < t->n_seq; q++) {
+        memcpy(out + pos, t->lit + lp, t->lit_len[q]);           /* literal run */
+        pos += t->lit_len[q]; lp += t->lit_len[q];
+        uint64_t src = t->src[q], ml = t->match_len[q];
+        if (src + ml > pos || pos + ml > end) return ORA_E_CORRUPT; /* strictly before */
+        memcpy(out + pos, out + src, ml);                         /* absolute-offset copy */
+        pos += ml;
+    }
+    memcpy(out + pos, t->lit + lp, t->trailing);
+    pos += t->trailing; lp += t->trailing;
+    if (lp != t->n_lit || pos != end) return ORA_E_CORRUPT;
+    return ORA_OK;
+}
+
 int ora_decode_all(const uint8_t *c, size_t clen, uint8_t *out, size_t cap)
 {
     ora_container k;
@@ -243,22 +262,38 @@ int ora_decode_all(const uint8_t *c, size_t clen, uint8_t *out, size_t cap)
     if (!t) return ORA_E_NOMEM;
     for (uint64_t b = 0; b < k.info.n_blocks && rc == ORA_OK; b++) {
         if ((rc = ora_tokens_decode(&k, b, t)) != ORA_OK) break;
-        uint64_t pos = b * ORA_B, end = pos + t->block_len;
-        uint32_t lp = 0;
-        for (uint32_t q = 0; q < t->n_seq; q++) {
-            memcpy(out + pos, t->lit + lp, t->lit_len[q]);           /* literal run */
-            pos += t->lit_len[q]; lp += t->lit_len[q];
-            uint64_t src = t->src[q], ml = t->match_len[q];
-            if (src + ml > pos || pos + ml > end) { rc = ORA_E_CORRUPT; break; } /* strictly before */
-            memcpy(out + pos, out + src, ml);                         /* absolute-offset copy */
-            pos += ml;
-        }
-        if (rc != ORA_OK) break;
-        memcpy(out + pos, t->lit + lp, t->trailing);
-        pos += t->trailing; lp += t->trailing;
-        if (lp != t->n_lit || pos != end) rc = ORA_E_CORRUPT;
+        rc = emit_block(t, b, out);
     }
     free(t);
+    return rc;
+}
+
+/* Decoder #1 with the entropy stage spread over host threads (SURVEY.md section 8d "oracle timed beside it",
+ * variant b): blocks are independent in the entropy layer, so groups of blocks are entropy-decoded
+ * and parsed in parallel (the same ora_tokens_decode per block); the match stage then emits them one after the
+ * other in block order, because a copy may read any earlier output byte. Same result as
+ * ora_decode_all by construction; pinned by tests/test_oracle_codec.py. */
+int ora_decode_all_mt(const uint8_t *c, size_t clen, uint8_t *out, size_t cap, uint32_t threads)
+{
+    ora_container k;
+    int rc = ora_container_open(c, clen, &k);
+    if (rc != ORA_OK) return rc;
+    if (cap < k.info.total_len) return ORA_E_CAPACITY;
+    if (threads < 1) threads = 1;
+    const uint64_t group = 4 * (uint64_t)threads;
+    ora_tokens *t = (ora_tokens *)malloc(sizeof *t * group);
+    int *rcs = (int *)malloc(sizeof *rcs * group);
+    if (!t || !rcs) { free(t); free(rcs); return ORA_E_NOMEM; }
+    for (uint64_t b0 = 0; b0 < k.info.n_blocks && rc == ORA_OK; b0 += group) {
+        const uint64_t n = k.info.n_blocks - b0 < group ? k.info.n_blocks - b0 : group;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads)
+        for (int64_t i = 0; i < (int64_t)n; i++) rcs[i] = ora_tokens_decode(&k, b0 + (uint64_t)i, &t[i]);
+        for (uint64_t i = 0; i < n && rc == ORA_OK; i++) {
+            rc = rcs[i];
+            if (rc == ORA_OK) rc = emit_block(&t[i], b0 + i, out);
+        }
+    }
+    free(t); free(rcs);
     return rc;
 }
 

@@ -214,7 +214,9 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
     if (rc != ACEAPEX_OK) { aceapex_close(c); return rc; }
 
     c->sl = make_slot_layout(res.max_n_seq, c->cv.W);
-    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem(c)) != cudaSuccess) {
+    // The attribute belongs to the function, not to this context: set it to the format maximum (4096 sequences,
+    // 8-byte offsets) so that contexts of different containers cannot lower each other's limit.
+    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem_bytes(kMaxSeq, 8)) != cudaSuccess) {
         aceapex_close(c);
         return ACEAPEX_E_CUDA;
     }

@@ -97,7 +97,7 @@ __host__ __device__ inline uint32_t match_smem_bytes(uint32_t ms, uint32_t W)
 {
     // delta (16 ms + 16), dm (4 ms), tlist (2 ms), staged LEN / slist (2 ms), staged OFF (W ms + 16: the
     // word-wise offset read may touch 11 bytes past the last offset), staged tags (ms / 2)
-    return kMatchFixedSmem + 16 * ms + 16 + 4 * ms + 2 * ms + 2 * ms + (W * ms + 16) + ms / 2;
+    return kMatchFixedSmem + 16 * ms + 16 + 4 * ms + 2 * ms + 2 * ms + (W * ms + 16) + ((ms / 2 + 15u) & ~15u);
 }
 
 __device__ inline uint32_t ldg_u8(unsigned long long a)
@@ -405,6 +405,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                         *reinterpret_cast<ulonglong2 *>(&delta[2 * k + 1]) = make_ulonglong2(lit_a + lp - st, out_a + src - d);
                         dm[k] = d | ml << 16;
                         if (src + ml > B0 + d) bad = true;             // strictly before, non-overlapping
+                        // FORMAT.md section 4: tag 0 iff the source range lies entirely below the block
+                        if ((tg == 0) != (src + ml <= B0)) bad = true;
                         // a source that starts in block sb < blk ends in block sb or sb + 1 (ml <= 16384)
                         const uint64_t sb = src >> kBlockLog2;
                         if (sb < blk) below = max(below, min((uint32_t)sb + 2u, blk32));
@@ -490,10 +492,13 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                     for (int u = 0; u < (int)kWordUnroll; u++) {
                         const unsigned long long wa = g[u].aA & ~3ull, wb = g[u].aB & ~3ull;
                         const uint32_t fa = (uint32_t)g[u].aA & 3u, fb = (uint32_t)g[u].aB & 3u, k = g[u].k;
+                        // a multi-boundary group takes the per-byte path below: its aB belongs to a run that starts
+                        // after byte k and may point up to 2 bytes before that run's source, i.e. before the buffer
+                        const bool useB = k < 4 && !g[u].multi;
                         alo[u] = ldg_u32(wa);
                         ahi[u] = fa + k > 4 ? ldg_u32(wa + 4) : 0u;            // k = 4 for a group inside one run
-                        blo[u] = k < 4 ? ldg_u32(wb) : 0u;
-                        bhi[u] = (k < 4 && fb + (4 - k) > 4) ? ldg_u32(wb + 4) : 0u;
+                        blo[u] = useB ? ldg_u32(wb) : 0u;
+                        bhi[u] = (useB && fb + (4 - k) > 4) ? ldg_u32(wb + 4) : 0u;
                     }
 #pragma unroll
                     for (int u = 0; u < (int)kWordUnroll; u++) {

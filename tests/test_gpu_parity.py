@@ -137,6 +137,47 @@ def test_configs_2_3_full_size(binding, name):
             assert np.array_equal(got[i * B:i * B + blk.size], blk), b
 
 
+def test_config4_mixed_1g_full_size(binding):
+    """BASELINE.json configs[4] at full size with the binding's defaults (one batch of 65,536 slots): decode_all
+    against the original bytes (round-trip identity pins decoder #1); the seeded 100,000 block ids as ONE
+    decode_blocks(PACKED) at n_targets=1024 (the group size bench.py times), every block compared with the original
+    (decoder #2 == decoder #1 == original is pinned on the CPU side); 2,048 individual aceapex_seek calls compared the
+    same way and 48 of them against oracle decoder #2 itself."""
+    cfg = W.CONFIGS["mixed_1g"]
+    data = cfg.data()
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=32, **cfg.encoder)
+    nb = int(oracle.info(c).n_blocks)
+    assert nb == 65536
+    d_data = torch.from_numpy(data).cuda()
+    with binding.Decoder(c, n_targets=1024) as dec:
+        assert dec.n_slots == 65536
+        out = dev_out(data.size)
+        dec.decode_all(out)
+        dec.check()
+        assert torch.equal(out, d_data)
+        del out
+        ids = W.seek_ids(nb, 100_000, W.SEED_BASE + 0x70 + 4)
+        bout = dev_out(len(ids) * B)
+        dec.decode_blocks(ids, bout)
+        dec.check()
+        idx = torch.from_numpy(ids.astype(np.int64)).cuda()
+        step = 10_000                                               # compare in slices: keeps the gather small
+        for i in range(0, len(ids), step):
+            want = d_data.view(nb, B)[idx[i:i + step]]
+            assert torch.equal(bout.view(-1, B)[i:i + step], want), i
+        del bout
+        dst = dev_out(B)
+        with oracle.Isolated(c) as iso:
+            for j, b in enumerate(ids[:2048]):
+                b = int(b)
+                _, start, blen = dec.seek(b * B + (j * 131) % B, dst)
+                assert (start, blen) == (b * B, B)
+                assert torch.equal(dst, d_data[b * B:(b + 1) * B]), b
+                if j < 48:
+                    assert np.array_equal(dst.cpu().numpy(), iso.decode(b)), b
+        dec.check()
+
+
 # ------------------------------------------------------------------ entropy layer alone
 
 @pytest.mark.parametrize("name", ["markov_1m", "genome_256m"])
@@ -203,6 +244,67 @@ def test_small_scratch_batches_and_slot_overflow(binding):
         want = oracle.decode_all(c)
         full_check(binding, c, want, n_slots=5, n_targets=2, seek_blocks=[40, 39, 17, 17, 3, 0])
         full_check(binding, c, want, n_slots=3, n_targets=1, seek_blocks=[33, 40])
+
+
+def test_multi_boundary_group_with_source_at_position_zero(binding):
+    """A 4-byte output group with two run boundaries whose last run is a match from absolute position 0: the
+    word-granular gather must not touch the bytes in front of the output buffer (the buffer is a fresh allocation)."""
+    lits0 = bytes((i * 13 + 1) & 0xFF for i in range(B))
+    # block 1: match(4) from 100 | 1 literal | match(4) from 0 | 2 literals | match(5) from 1 | rest literals
+    seqs1 = [(0, 4, 100), (1, 4, 0), (2, 5, 1), (1, 4, 0), (1, 4, 1)]
+    nlit1 = B - sum(ml for _, ml, _ in seqs1)
+    lits1 = bytes((i * 7 + 5) & 0xFF for i in range(nlit1))
+    blocks = [([], lits0), (seqs1, lits1)]
+    want = np.frombuffer(expand(2 * B, blocks), np.uint8)
+    c = container_from_tokens(2 * B, blocks)
+    assert np.array_equal(oracle.decode_all(c), want)
+    torch.cuda.empty_cache()
+    with binding.Decoder(c, n_targets=2) as dec:
+        out = torch.full((64 << 20,), 0xA5, dtype=torch.uint8, device="cuda")   # its own segment: nothing mapped in front is ours
+        dec.decode_all(out)
+        dec.check()
+        assert np.array_equal(out[:2 * B].cpu().numpy(), want)
+        assert bool((out[2 * B:] == 0xA5).all())
+        got = dec.decode_blocks(np.array([1, 0], np.uint64), dev_out(2 * B)).cpu().numpy()
+        dec.check()
+        assert np.array_equal(got[:B], want[B:]) and np.array_equal(got[B:], want[:B])
+
+
+def test_two_open_decoders_of_different_containers(binding):
+    """Two live contexts whose containers need different amounts of match-kernel shared memory (config 0 under the
+    literal policy has thousands of sequences per block, FASTQ a few hundred) must not disturb each other."""
+    big = W.CONFIGS["markov_1m"].data(8 * B)
+    c_big = oracle.encode(big, **W.POLICY_LITERAL)
+    small = W.generate("fastq", 8 * B + 5, 3)
+    c_small = oracle.encode(small, min_match=8, max_depth=8, window=2, batch=2)
+    with binding.Decoder(c_big, n_targets=2) as d_big:
+        o1 = dev_out(big.size)
+        d_big.decode_all(o1); d_big.check()
+        with binding.Decoder(c_small, n_targets=2) as d_small:
+            assert d_small.info.max_n_seq < d_big.info.max_n_seq
+            o2 = dev_out(small.size)
+            d_small.decode_all(o2); d_small.check()
+            o1.fill_(0xA5)
+            d_big.decode_all(o1); d_big.check()                  # after the smaller container was opened
+            o2.fill_(0xA5)
+            d_small.decode_all(o2); d_small.check()
+            assert np.array_equal(o2.cpu().numpy(), small)
+        assert np.array_equal(o1.cpu().numpy(), big)
+
+
+def test_rejects_inconsistent_tag(binding):
+    """FORMAT.md section 4: tag 0 iff the source range lies entirely below the block. A match tagged 0 whose source
+    reaches into its own block (it would read bytes that pass 0 has not produced yet) is reported, not decoded."""
+    lits = b"abcdefgh" + b"z" * (B - 16)
+    rec = build_record(0, [(8, 8, 0)], lits, tags=[0])              # in-block source, tag says cross-block
+    expect_corrupt(binding, build_container(B, [rec]), B, 0)
+    lits0 = bytes(range(256)) * (B // 256)
+    rec0 = build_record(0, [], lits0)
+    rec1 = build_record(B, [(8, 8, 16)], lits, tags=[1])            # source entirely below the block, tag says in-block
+    with binding.Decoder(build_container(2 * B, [rec0, rec1]), n_targets=1) as dec:
+        dec.decode_all(dev_out(2 * B))
+        rc, first = dec.device_status(clear=True)
+        assert rc == binding.E_CORRUPT and first == 1
 
 
 # ------------------------------------------------------------------ isolation (PAPER.md:45-51)

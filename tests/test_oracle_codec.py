@@ -76,6 +76,7 @@ def test_round_trip_adversarial(name, policy):
     params = dict(min_match=4) if policy == "literal" else dict(min_match=8, max_depth=3, window=2, batch=2, threads=3)
     c = oracle.encode(data, **params)
     assert oracle.decode_all(c).tobytes() == data
+    assert oracle.decode_all_mt(c, 4).tobytes() == data
     i = oracle.info(c)
     assert i.total_len == len(data) and i.n_blocks == (len(data) + B - 1) // B
     assert i.container_bytes == c.size
@@ -141,6 +142,8 @@ def test_profiles_round_trip_and_decoders_agree(name, nbytes, policy):
     full = oracle.decode_all(c)
     assert np.array_equal(full, data)
     assert oracle.fnv1a64(full) == oracle.fnv1a64(data)            # PAPER.md:41 FNV check
+    for threads in (1, 3):                                           # multi-core driver of the same decoder
+        assert np.array_equal(oracle.decode_all_mt(c, threads), data)
     rep = oracle.validate(c)                                         # src+len<=dst, tags, D, R
     assert rep.n_matches_cross + rep.n_matches_intra + rep.n_matches_spanning == rep.n_seq
     if params.get("max_depth"):
@@ -213,6 +216,8 @@ def test_rejects_bad_frequency_sum_and_length_mismatch():
     bad[p] ^= 1
     with pytest.raises(oracle.OracleError):
         oracle.decode_all(bad)
+    with pytest.raises(oracle.OracleError):
+        oracle.decode_all_mt(bad, 3)
     # block whose tokens do not add up to the block length
     rec = build_record(0, [(8, 8, 0)], b"ABCDEFGH" + b"q" * 10)
     with pytest.raises(oracle.OracleError):
