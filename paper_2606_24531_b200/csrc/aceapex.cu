@@ -293,7 +293,7 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
         if (cudaMemsetAsync(c->sc.done, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
         c->epoch = 1;
     }
-    const uint32_t aligned = ((uintptr_t)d_out & 3) == 0;
+    const uint32_t aligned = ((uintptr_t)d_out & 15) == 0 ? 16u : (((uintptr_t)d_out & 3) == 0 ? 4u : 1u);
     for (uint64_t first = 0; first < c->cv.n_blocks; first += c->sc.n_slots) {
         const uint64_t rest = c->cv.n_blocks - first;
         const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);
@@ -447,16 +447,6 @@ int aceapex_profile_read(aceapex_ctx *c, uint64_t *launches, double *ms)
     c->prof_recs.clear();
     return rc;
 }
-
-#ifdef ACEAPEX_TRACE
-int aceapex_debug_trace(unsigned long long *out16, int reset)
-{
-    cudaDeviceSynchronize();
-    if (out16) cudaMemcpyFromSymbol(out16, g_trace, sizeof(unsigned long long) * 16);
-    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(g_trace, z, sizeof z); }
-    return 0;
-}
-#endif
 
 const char *aceapex_kernel_name(int id) { return id >= 0 && id < K_COUNT ? kKernelNames[id] : nullptr; }
 

@@ -264,12 +264,6 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
     const uint64_t n_thr = (uint64_t)n_ctas * blockDim.x, gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t n_warps = n_ctas * kEntropyWarps, gwarp = blockIdx.x * kEntropyWarps + warp;
     const uint64_t n_bytes = (uint64_t)a.nt * kB;
-#ifdef ACEAPEX_TRACE
-    long long st_prev = clock64();
-#define SEEK_MARK(i) do { if (gtid == 0) { const long long t_ = clock64(); atomicAdd(&g_trace[i], (unsigned long long)(t_ - st_prev)); st_prev = t_; } } while (0)
-#else
-#define SEEK_MARK(i) do { } while (0)
-#endif
 
     // init: every target byte chases its own position
     for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
@@ -293,13 +287,8 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
         grid_barrier(ctl, n_ctas);
         for (;; hop++) {
             const uint32_t hp = hop & 1u;
-            SEEK_MARK(10);
             const uint32_t n_claimed = ld_acquire_u32(&ctl->round_n_list[rp]);
             const uint32_t n_now = n_claimed < a.max_slots ? n_claimed : a.max_slots;
-            SEEK_MARK(11);
-#ifdef ACEAPEX_TRACE
-            if (gtid == 0) atomicAdd(&g_trace[15], 1ull);
-#endif
             // ---- entropy: LEN and OFF of the new blocks, warp per (block, stream) unit
             const uint32_t n_new = n_now - n_ready;
             for (uint32_t u = gwarp; u < 2 * n_new; u += n_warps) {
@@ -312,7 +301,6 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
                 ctl->hop_pending[hp ^ 1u] = 0;
                 if (n_ready == 0) ctl->round_n_list[rp ^ 1u] = 0;
             }
-            SEEK_MARK(12);
             // ---- parse the new blocks, four warps per block
             for (uint32_t b0 = n_ready + blockIdx.x * (kEntropyWarps / 4); b0 < n_now; b0 += n_ctas * (kEntropyWarps / 4)) {
                 const uint32_t bi = b0 + (warp >> 2);
@@ -320,7 +308,6 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
                 quad_parse_block(cv, sl, slot, slot ? a.list[bi] : 0, ctl, lane, warp & 3u, s_quad[warp >> 2]);
             }
             grid_barrier(ctl, n_ctas);
-            SEEK_MARK(13);
             n_ready = n_now;
             // ---- chase every byte through the resident blocks
             if (threadIdx.x == 0) s_rem = 0;
@@ -339,7 +326,6 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
             if (threadIdx.x == 0 && s_rem) atomicAdd(&ctl->hop_pending[hp], (unsigned long long)s_rem);
             grid_barrier(ctl, n_ctas);
             chasing = ctl->hop_pending[hp];
-            SEEK_MARK(14);
             // out of slots: the blocks claimed beyond max_slots wait for the next round
             if (chasing == 0 || n_claimed >= a.max_slots || hop + 1 >= a.max_hops) { hop++; break; }
         }
@@ -349,7 +335,6 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
             if (h->need_lit && h->parsed_ok) decode_unit(cv, sl, a.slots, a.list[bi], bi, LIT, false, ws, lane, ctl);
         }
         grid_barrier(ctl, n_ctas);
-        SEEK_MARK(8);
         for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
             const unsigned long long p = a.pend[g];
             if (p == kDone || p < kLitReq) continue;

@@ -18,6 +18,7 @@ def test_reference_arm_prints_one_json_line():
     assert d["impl"] == "reference" and d["unit"] == "GB/s" and d["higher_is_better"] is True
     assert d["metric"] == "two_layer_decode_GBps_decompressed" and d["value"] > 0 and d["steps"] == 2
     assert d["config"]["workload"] == "markov_1m" and d["config"]["bytes"] == 3 * 16384 + 11
-    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == (os.cpu_count() or 1)
+    assert d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
     assert d["vs_baseline"] is None and d["dtype"] == "u8" and d["data"] == "synthetic"

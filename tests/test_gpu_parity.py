@@ -297,7 +297,15 @@ def test_rejects_inconsistent_tag(binding):
     reaches into its own block (it would read bytes that pass 0 has not produced yet) is reported, not decoded."""
     lits = b"abcdefgh" + b"z" * (B - 16)
     rec = build_record(0, [(8, 8, 0)], lits, tags=[0])              # in-block source, tag says cross-block
-    expect_corrupt(binding, build_container(B, [rec]), B, 0)
+    with binding.Decoder(build_container(B, [rec]), n_targets=1) as dec:
+        out = dev_out(B + 64)
+        dec.decode_all(out)
+        rc, first = dec.device_status(clear=True)
+        assert rc == binding.E_CORRUPT and first == 0
+        assert bool((out == 0xA5).all())                             # the bad block is left unwritten
+        # the isolated path never uses tags (scheduling metadata): it returns the right bytes
+        got = dec.decode_blocks(np.array([0], np.uint64), dev_out(B)).cpu().numpy()
+        assert dec.device_status()[0] == 0 and got[:16].tobytes() == b"abcdefghabcdefgh"
     lits0 = bytes(range(256)) * (B // 256)
     rec0 = build_record(0, [], lits0)
     rec1 = build_record(B, [(8, 8, 16)], lits, tags=[1])            # source entirely below the block, tag says in-block
