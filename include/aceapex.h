@@ -21,9 +21,10 @@
  *     position, ...) never cause an out-of-bounds access: the offending block is left
  *     unwritten, a sticky status word is set in device memory and aceapex_device_status()
  *     returns ACEAPEX_E_CORRUPT.
- *   - Every decode call is asynchronous on `cuda_stream`: decode_all enqueues two kernels per
- *     batch of n_slots blocks, decode_blocks / seek one fused kernel per group of n_targets
- *     blocks (the copy-hop loop runs on the device and ends there; no host read-back).
+ *   - Every decode call is asynchronous on `cuda_stream`: decode_all / decode_range enqueue two
+ *     kernels per batch of n_slots blocks (decode_range with first > 0: three), decode_blocks / seek
+ *     one fused kernel per group of n_targets blocks (the copy-hop loop runs on the device and ends
+ *     there; no host read-back).
  *   - There is no CPU fallback: without a CUDA device every call except aceapex_strerror and
  *     aceapex_version fails with ACEAPEX_E_CUDA.
  */
@@ -110,6 +111,20 @@ int aceapex_set_scratch(aceapex_ctx *ctx, void *d_scratch, size_t nbytes, size_t
  * copies from earlier blocks waits until those are complete ("any block decodes
  * once the blocks holding its source bytes are present"). */
 int aceapex_decode_all(aceapex_ctx *ctx, void *d_out, size_t out_capacity, void *cuda_stream);
+
+/* Range decode ("makes range decoding mandatory rather than optional": blocks 0-1000 of a 3 M block
+ * archive; a file decoded in sub-batches): blocks [first, first + count) through both layers into a
+ * RANGE-SIZED buffer, block first + i at d_out + i * 16384; writes d_out[0, (count-1)*16384 + block_len(last)) and
+ * nothing else.
+ *   first, count  blocks; first + count <= n_blocks (else ACEAPEX_E_RANGE); count == 0 is a no-op.
+ *   d_out         DEVICE, capacity `out_capacity` >= the bytes written (else ACEAPEX_E_CAPACITY).
+ * The range runs through the same entropy and match kernels as aceapex_decode_all, in sub-batches of
+ * min(n_slots, n_targets) blocks. Copies whose source starts below block `first` cannot be taken from the buffer:
+ * exactly those bytes are first followed to their origins through the compressed data (the isolated path of
+ * aceapex_decode_blocks, restricted to them) and written in place; needs n_targets >= 1 in the scratch when
+ * first > 0 (else ACEAPEX_E_STATE). Asynchronous on `cuda_stream`. */
+int aceapex_decode_range(aceapex_ctx *ctx, uint64_t first, uint64_t count, void *d_out, size_t out_capacity,
+                         void *cuda_stream);
 
 /* Isolated decode of the listed blocks.
  *   h_ids  HOST, n_ids block ids, each < n_blocks (else ACEAPEX_E_RANGE); duplicates allowed.

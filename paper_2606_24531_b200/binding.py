@@ -23,7 +23,7 @@ E_ARG, E_FORMAT, E_CAPACITY, E_CORRUPT, E_RANGE, E_NOMEM, E_CUDA, E_STATE = -1, 
 
 # every symbol include/aceapex.h declares
 SYMBOLS = ["aceapex_version", "aceapex_open", "aceapex_info_get", "aceapex_scratch_bytes", "aceapex_set_scratch",
-           "aceapex_decode_all", "aceapex_decode_blocks", "aceapex_seek", "aceapex_device_status",
+           "aceapex_decode_all", "aceapex_decode_range", "aceapex_decode_blocks", "aceapex_seek", "aceapex_device_status",
            "aceapex_launch_count", "aceapex_decode_streams", "aceapex_profile_enable", "aceapex_profile_read",
            "aceapex_kernel_name", "aceapex_strerror", "aceapex_close"]
 N_KERNELS = 16
@@ -63,6 +63,7 @@ def lib():
             L.aceapex_scratch_bytes.argtypes = [vp, sz, sz]; L.aceapex_scratch_bytes.restype = sz
             L.aceapex_set_scratch.argtypes = [vp, vp, sz, sz, sz, vp]
             L.aceapex_decode_all.argtypes = [vp, vp, sz, vp]
+            L.aceapex_decode_range.argtypes = [vp, u64, u64, vp, sz, vp]
             L.aceapex_decode_blocks.argtypes = [vp, vp, sz, vp, sz, u32, vp]
             L.aceapex_seek.argtypes = [vp, u64, vp, sz, C.POINTER(u64), C.POINTER(u32), vp]
             L.aceapex_device_status.argtypes = [vp, vp, C.POINTER(u64), C.c_int]
@@ -135,6 +136,17 @@ class Decoder:
             out = torch.empty(max(1, int(self.info.total_len)), dtype=torch.uint8, device=self.device)
         with torch.cuda.device(self.device):
             _check(lib().aceapex_decode_all(self._ctx, out.data_ptr(), out.numel(), _stream_ptr(stream)), "aceapex_decode_all")
+        return out
+
+    # -- aceapex_decode_range
+    def decode_range(self, first: int, count: int, out=None, stream=None):
+        """Blocks [first, first+count) into a range-sized buffer (block first+i at out[i*16384:])."""
+        torch = self._torch
+        if out is None:
+            out = torch.empty(max(1, count * B), dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            _check(lib().aceapex_decode_range(self._ctx, int(first), int(count), out.data_ptr(), out.numel(),
+                                              _stream_ptr(stream)), "aceapex_decode_range")
         return out
 
     # -- aceapex_decode_blocks

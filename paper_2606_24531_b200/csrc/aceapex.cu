@@ -107,7 +107,7 @@ uint32_t match_grid(aceapex_ctx *c, uint32_t count)
 }
 
 int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list, uint32_t max_slots, uint64_t first,
-                   uint32_t count, cudaStream_t st, uint32_t reset_watermark = 0)
+                   uint32_t count, cudaStream_t st, uint32_t reset_watermark = 0, uint64_t wm_init = 0)
 {
     uint32_t units = 3 * (list ? max_slots : count);
     uint32_t grid = (units + kEntropyWarps - 1) / kEntropyWarps;
@@ -117,9 +117,90 @@ int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list,
     {
         LaunchScope ls(c, K_ENTROPY, st);
         k_entropy<<<grid, 32 * kEntropyWarps, entropy_smem(), st>>>(c->cv, c->sl, c->sc.slots, list, n_list, max_slots, first, count,
-                                                     c->sc.ctl, reset_watermark);
+                                                     c->sc.ctl, reset_watermark, (unsigned long long)wm_init);
     }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
+}
+
+// One group of at most n_targets blocks through the fused isolated-decode kernel. `h_ids` == nullptr: the
+// consecutive blocks id0, id0 + 1, ... (range mode when range_lo_blocks > 0: see seek.cuh chase_byte).
+int launch_seek_group(aceapex_ctx *c, const uint64_t *h_ids, uint64_t id0, uint32_t nt, uint8_t *d_out, uint64_t out_base,
+                      bool absolute, bool range_mode, uint64_t range_lo, cudaStream_t st)
+{
+    const uint32_t S = (uint32_t)(c->sc.n_slots > 0xFFFFFFFFull / 4 ? 0xFFFFFFFFull / 4 : c->sc.n_slots);
+    if (c->seek_ctas_per_sm == 0) {
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_seek_fused, 32 * (int)kEntropyWarps, entropy_smem()) != cudaSuccess || nb < 1)
+            return ACEAPEX_E_CUDA;
+        c->seek_ctas_per_sm = nb;
+    }
+    const uint32_t kMaxHops = 1u << 16;
+    if (c->tag > 0xFFFFFFFFu - 2 * kMaxHops) {                         // hop tags would wrap: start over
+        if (cudaMemsetAsync(c->sc.mark, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        c->tag = 0;
+    }
+    SeekArgs a;
+    a.pend = c->sc.pend; a.mark = c->sc.mark; a.slot_of = c->sc.slot_of; a.list = c->sc.list;
+    a.slots = c->sc.slots; a.out = d_out;
+    a.out_base = out_base; a.nt = nt; a.absolute = absolute ? 1u : 0u; a.max_slots = S;
+    a.tag0 = c->tag + 1; a.max_hops = kMaxHops;
+    a.range_mode = range_mode ? 1u : 0u; a.range_lo = range_lo;
+    c->tag += kMaxHops;
+    if (!h_ids || nt == 1) {
+        a.ids = nullptr; a.one_id = h_ids ? h_ids[0] : id0;            // consecutive targets need no copy at all
+    } else {
+        if (cudaMemcpyAsync(c->sc.ids, h_ids, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        a.ids = c->sc.ids; a.one_id = 0;
+    }
+    // all CTAs must be co-resident (grid barrier): one CTA per SM for a few targets (cheaper
+    // barriers), the full occupancy for batches
+    uint32_t grid = (uint32_t)c->sm_count * (nt <= 4 ? 1u : (uint32_t)c->seek_ctas_per_sm);
+    Control *ctl = c->sc.ctl;
+    void *params[] = { &c->cv, &c->sl, &a, &ctl };
+    {
+        LaunchScope ls(c, K_SEEK_FUSED, st);
+        if (cudaLaunchCooperativeKernel((const void *)k_seek_fused, dim3(grid), dim3(32 * kEntropyWarps), params, entropy_smem(), st) !=
+            cudaSuccess)
+            return ACEAPEX_E_CUDA;
+    }
+    return ACEAPEX_OK;
+}
+
+// Blocks [first, first + count) through both layers into d_out (block first + i at d_out + i * 16384), in
+// sub-batches of the scratch's slot count (PAPER.md:112 decodes a whole file in sub-batches). first == 0 with
+// count == n_blocks is decode_all. For first > 0 (PAPER.md:104 range decode) the sources that lie below the
+// range are not in the buffer: before a sub-batch is entropy-decoded and matched, the fused isolated kernel
+// follows exactly those bytes to their origins through the compressed data and writes them in place; the match
+// kernel then takes every other byte from the range's own buffer.
+int decode_span(aceapex_ctx *c, uint64_t first, uint64_t count, uint8_t *d_out, cudaStream_t st)
+{
+    if (++c->epoch == 0) {   // epoch wrapped: stale done flags could alias
+        if (cudaMemsetAsync(c->sc.done, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        c->epoch = 1;
+    }
+    const uint32_t align = ((uintptr_t)d_out & 15) == 0 ? 16u : (((uintptr_t)d_out & 3) == 0 ? 4u : 1u);
+    const uint64_t range_lo = first << kBlockLog2;
+    uint8_t *out_virtual = d_out - range_lo;                           // absolute output offset -> address
+    uint64_t step = c->sc.n_slots;
+    if (first > 0 && c->sc.n_targets < step) step = c->sc.n_targets;
+    for (uint64_t f = first; f < first + count; f += step) {
+        const uint64_t rest = first + count - f;
+        const uint32_t cnt = (uint32_t)(rest < step ? rest : step);
+        if (first > 0) {
+            int rc = launch_seek_group(c, nullptr, f, cnt, d_out, f - first, false, true, range_lo, st);
+            if (rc != ACEAPEX_OK) return rc;
+        }
+        // the first entropy launch of the call also re-arms the watermark (nothing reads it before the match kernel)
+        int rc = launch_entropy(c, nullptr, nullptr, 0, f, cnt, st, f == first ? 1u : 0u, first);
+        if (rc != ACEAPEX_OK) return rc;
+        {
+            LaunchScope ls(c, K_MATCH, st);
+            k_match<<<match_grid(c, cnt), kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, f, cnt, out_virtual, align,
+                                                                    c->sc.ctl, c->sc.done, c->epoch, range_lo);
+        }
+        if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
+    }
+    return ACEAPEX_OK;
 }
 
 }  // namespace
@@ -288,27 +369,19 @@ int aceapex_decode_all(aceapex_ctx *c, void *d_out, size_t out_capacity, void *c
     if (!c->have_scratch) return ACEAPEX_E_STATE;
     if (out_capacity < c->info.total_len) return ACEAPEX_E_CAPACITY;
     if (c->cv.n_blocks == 0) return ACEAPEX_OK;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (++c->epoch == 0) {   // epoch wrapped: stale done flags could alias
-        if (cudaMemsetAsync(c->sc.done, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-        c->epoch = 1;
-    }
-    const uint32_t aligned = ((uintptr_t)d_out & 15) == 0 ? 16u : (((uintptr_t)d_out & 3) == 0 ? 4u : 1u);
-    for (uint64_t first = 0; first < c->cv.n_blocks; first += c->sc.n_slots) {
-        const uint64_t rest = c->cv.n_blocks - first;
-        const uint32_t count = (uint32_t)(rest < c->sc.n_slots ? rest : c->sc.n_slots);
-        // the first entropy launch of the call also resets the watermark (nothing reads it before the match kernel)
-        int rc = launch_entropy(c, nullptr, nullptr, 0, first, count, st, first == 0 ? 1u : 0u);
-        if (rc != ACEAPEX_OK) return rc;
-        {
-            LaunchScope ls(c, K_MATCH, st);
-            k_match<<<match_grid(c, count), kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, first, count,
-                                                                    static_cast<uint8_t *>(d_out), aligned, c->sc.ctl,
-                                                                    c->sc.done, c->epoch);
-        }
-        if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
-    }
-    return ACEAPEX_OK;
+    return decode_span(c, 0, c->cv.n_blocks, static_cast<uint8_t *>(d_out), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int aceapex_decode_range(aceapex_ctx *c, uint64_t first, uint64_t count, void *d_out, size_t out_capacity, void *cuda_stream)
+{
+    if (!c || (count && !d_out)) return ACEAPEX_E_ARG;
+    if (first + count < first || first + count > c->cv.n_blocks) return ACEAPEX_E_RANGE;
+    if (count == 0) return ACEAPEX_OK;
+    if (!c->have_scratch || (first > 0 && c->sc.n_targets == 0)) return ACEAPEX_E_STATE;
+    const uint64_t last = first + count - 1;
+    const size_t need = (size_t)((count - 1) << kBlockLog2) + block_len_host(c, last);
+    if (out_capacity < need) return ACEAPEX_E_CAPACITY;
+    return decode_span(c, first, count, static_cast<uint8_t *>(d_out), static_cast<cudaStream_t>(cuda_stream));
 }
 
 int aceapex_decode_streams(aceapex_ctx *c, uint64_t first, size_t count, void *d_lit, void *d_len, void *d_off,
@@ -346,45 +419,10 @@ int aceapex_decode_blocks(aceapex_ctx *c, const uint64_t *h_ids, size_t n_ids, v
     }
     if (out_capacity < need) return ACEAPEX_E_CAPACITY;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const uint32_t S = (uint32_t)(c->sc.n_slots > 0xFFFFFFFFull / 4 ? 0xFFFFFFFFull / 4 : c->sc.n_slots);
-    if (c->seek_ctas_per_sm == 0) {
-        int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_seek_fused, 32 * (int)kEntropyWarps, entropy_smem()) != cudaSuccess || nb < 1)
-            return ACEAPEX_E_CUDA;
-        c->seek_ctas_per_sm = nb;
-    }
-    const uint32_t kMaxHops = 1u << 16;
-
     for (size_t base = 0; base < n_ids; base += c->sc.n_targets) {
         const uint32_t nt = (uint32_t)(n_ids - base < c->sc.n_targets ? n_ids - base : c->sc.n_targets);
-        if (c->tag > 0xFFFFFFFFu - 2 * kMaxHops) {                     // hop tags would wrap: start over
-            if (cudaMemsetAsync(c->sc.mark, 0, 4 * (size_t)c->cv.n_blocks, st) != cudaSuccess) return ACEAPEX_E_CUDA;
-            c->tag = 0;
-        }
-        SeekArgs a;
-        a.pend = c->sc.pend; a.mark = c->sc.mark; a.slot_of = c->sc.slot_of; a.list = c->sc.list;
-        a.slots = c->sc.slots; a.out = static_cast<uint8_t *>(d_out);
-        a.out_base = (uint64_t)base; a.nt = nt; a.absolute = absolute ? 1u : 0u; a.max_slots = S;
-        a.tag0 = c->tag + 1; a.max_hops = kMaxHops;
-        c->tag += kMaxHops;
-        if (nt == 1) {
-            a.ids = nullptr; a.one_id = h_ids[base];                   // a single seek needs no copy at all
-        } else {
-            if (cudaMemcpyAsync(c->sc.ids, h_ids + base, 8 * (size_t)nt, cudaMemcpyHostToDevice, st) != cudaSuccess)
-                return ACEAPEX_E_CUDA;
-            a.ids = c->sc.ids; a.one_id = 0;
-        }
-        // all CTAs must be co-resident (grid barrier): one CTA per SM for a few targets (cheaper
-        // barriers), the full occupancy for batches
-        uint32_t grid = (uint32_t)c->sm_count * (nt <= 4 ? 1u : (uint32_t)c->seek_ctas_per_sm);
-        Control *ctl = c->sc.ctl;
-        void *params[] = { &c->cv, &c->sl, &a, &ctl };
-        {
-            LaunchScope ls(c, K_SEEK_FUSED, st);
-            if (cudaLaunchCooperativeKernel((const void *)k_seek_fused, dim3(grid), dim3(32 * kEntropyWarps), params, entropy_smem(), st) !=
-                cudaSuccess)
-                return ACEAPEX_E_CUDA;
-        }
+        int rc = launch_seek_group(c, h_ids + base, 0, nt, static_cast<uint8_t *>(d_out), (uint64_t)base, absolute, false, 0, st);
+        if (rc != ACEAPEX_OK) return rc;
     }
     return cudaGetLastError() == cudaSuccess ? ACEAPEX_OK : ACEAPEX_E_CUDA;
 }

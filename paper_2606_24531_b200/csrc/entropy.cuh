@@ -313,11 +313,12 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
 // Unit u -> stream u / nb in the order LIT, OFF, LEN; block index u % nb (= slot). Output: the slot's areas.
 __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, SlotLayout sl, uint8_t *slots, const uint64_t *list,
                                                  const uint32_t *n_list, uint32_t max_slots, uint64_t first,
-                                                 uint32_t count, Control *ctl, uint32_t reset_watermark)
+                                                 uint32_t count, Control *ctl, uint32_t reset_watermark, unsigned long long wm_init)
 {
     extern __shared__ __align__(1024) uint8_t smem_entropy[];
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-    if (reset_watermark && blockIdx.x == 0 && threadIdx.x == 0) ctl->watermark = 0;   // decode_all: first launch of a call
+    // decode_all / decode_range: the first launch of a call re-arms the watermark (0, resp. the first block of the range)
+    if (reset_watermark && blockIdx.x == 0 && threadIdx.x == 0) ctl->watermark = wm_init;
     WarpSmem ws;
     {
         const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(smem_entropy);

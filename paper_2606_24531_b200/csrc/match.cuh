@@ -220,7 +220,7 @@ __device__ inline void stg_v4(unsigned long long a, uint4 v)
 __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayout sl, const uint8_t *slots,
                                                           uint64_t first, uint32_t count, uint8_t *out,
                                                           uint32_t out_align /* 16, 4 or 1 */, Control *ctl, uint32_t *done,
-                                                          uint32_t epoch)
+                                                          uint32_t epoch, uint64_t range_lo)
 {
     extern __shared__ __align__(16) uint8_t smem[];
     __shared__ uint32_t ws4[kMatchWarps][4];
@@ -437,14 +437,17 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                             atomicOr(&cb[d >> 5].x, bD);
                         }
                         if (ll) delta[rl] = lit_a + lp - st;
-                        delta[rm] = out_a + src - d;
+                        // Range decode: a source below the range is not in the buffer; the isolated
+                        // chase has already put this match's bytes in place, so the run copies itself onto itself.
+                        const bool ext = src < range_lo;
+                        delta[rm] = ext ? out_a + B0 : out_a + src - d;
                         dm[k] = d | ml << 16;
                         mrun[k] = (uint16_t)rm;
                         const uint64_t se = src + ml;
                         if (se > B0 + d) bad = true;                   // strictly before, non-overlapping
                         // FORMAT.md section 4: tag 0 iff the source range lies entirely below the block
                         if ((tg == 0) != (se <= B0)) bad = true;
-                        if (src < B0) last = max(last, min((unsigned long long)se, (unsigned long long)B0));
+                        if (!ext && src < B0) last = max(last, min((unsigned long long)se, (unsigned long long)B0));
                     }
                     const uint32_t tm = __ballot_sync(0xFFFFFFFFu, tg != 0);
                     if (tm) {                                          // warp-aggregated append to the tag list

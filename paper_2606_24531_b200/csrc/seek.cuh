@@ -169,19 +169,21 @@ struct SeekArgs {
     uint32_t *mark;          // [n_blocks] claim word: the tag of the round that claimed the block
     unsigned long long *slot_of;   // [n_blocks] tag << 32 | slot, written by the claimer right after it won
     uint64_t *list;
-    const uint64_t *ids;     // nt target ids (device); nullptr: the single target `one_id`
+    const uint64_t *ids;     // nt target ids (device); nullptr: the consecutive targets one_id, one_id + 1, ...
     uint64_t one_id;
+    uint64_t range_lo;       // range mode: first byte of the range being decoded (see chase_byte)
     uint8_t *slots;
     uint8_t *out;
     uint64_t out_base;       // packed mode: target i lands at out + (out_base + i) * 16384
     uint32_t nt, absolute, max_slots;
     uint32_t tag0;           // round r marks the blocks it claims with tag0 + r
     uint32_t max_hops;
+    uint32_t range_mode;     // 1: only bytes whose match source starts below range_lo are chased and written
 };
 
 constexpr unsigned long long kLitReq = 1ull << 62;   // pend = kLitReq | slot << 14 | index into the slot's LIT stream
 
-__device__ inline uint64_t seek_target(const SeekArgs &a, uint32_t i) { return a.ids ? a.ids[i] : a.one_id; }
+__device__ inline uint64_t seek_target(const SeekArgs &a, uint32_t i) { return a.ids ? a.ids[i] : a.one_id + i; }
 
 // Claim a slot of round `tag` for block blk (once: the claim word decides the winner). The slot entry
 // carries the tag, so a reader can never pair a fresh claim with a stale slot index.
@@ -200,9 +202,15 @@ __device__ inline void claim_block(const SeekArgs &a, Control *ctl, uint32_t tag
 // spot, for the next hop) or hits an inconsistency (-> kDone + status). Entries written during the
 // current phase have an index >= n_ready, and a stale cached entry can only carry an older tag: both
 // read as "not resident", which is always safe.
+//
+// Range mode (aceapex_decode_range): the targets are the consecutive blocks of a range whose other
+// bytes the match kernel produces from the output buffer. A byte still at its OWN position (`own`) is at its first
+// step: a literal, or a match whose source starts at or above range_lo, is left to the match kernel (kDone, nothing
+// is written); a match whose source starts below the range is followed to its origin like any isolated byte.
 __device__ inline unsigned long long chase_byte(const SlotLayout &sl, const SeekArgs &a, Control *ctl, uint32_t tag,
-                                                uint32_t rp, uint32_t n_ready, unsigned long long p)
+                                                uint32_t rp, uint32_t n_ready, unsigned long long p, unsigned long long own)
 {
+    bool first_step = a.range_mode && p == own;
     for (;;) {
         const uint64_t blk = p >> kBlockLog2;
         const uint32_t o = (uint32_t)(p & (kB - 1));
@@ -223,12 +231,16 @@ __device__ inline unsigned long long chase_byte(const SlotLayout &sl, const Seek
         const uint32_t q = lo, st = start[q];
         const uint32_t d = q < n ? reinterpret_cast<const uint16_t *>(slot + sl.o_dst)[q] : blen;
         if (o < d) {                                                   // a literal: the origin
+            if (first_step) return kDone;
             const uint32_t li = (uint32_t)reinterpret_cast<const uint16_t *>(slot + sl.o_litpos)[q] + (o - st);
             if (li >= kB) { raise(ctl, kStChase, blk); return kDone; }
             h->need_lit = 1;
             return kLitReq | (unsigned long long)s << kBlockLog2 | li;
         }
-        const unsigned long long nxt = reinterpret_cast<const uint64_t *>(slot + sl.o_src)[q] + (o - d);   // a match
+        const unsigned long long src = reinterpret_cast<const uint64_t *>(slot + sl.o_src)[q];
+        if (first_step && src >= a.range_lo) return kDone;
+        first_step = false;
+        const unsigned long long nxt = src + (o - d);                 // a match
         if (nxt >= p) { raise(ctl, kStChase, blk); return kDone; }
         p = nxt;
     }
@@ -316,7 +328,8 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
             for (uint64_t g = gtid; g < n_bytes; g += n_thr) {
                 const unsigned long long p = a.pend[g];
                 if (p >= kLitReq) continue;
-                const unsigned long long q = chase_byte(sl, a, ctl, tag, rp, n_ready, p);
+                const unsigned long long own = (seek_target(a, (uint32_t)(g >> kBlockLog2)) << kBlockLog2) + (g & (kB - 1));
+                const unsigned long long q = chase_byte(sl, a, ctl, tag, rp, n_ready, p, own);
                 if (q != p) a.pend[g] = q;
                 remaining += q < kLitReq;
             }

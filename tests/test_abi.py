@@ -48,6 +48,7 @@ def test_calls_that_need_no_device():
     assert L.aceapex_open(16, 100, None, None) == binding.E_ARG
     assert L.aceapex_open(24, 4096, None, C.byref(ctx)) == binding.E_ARG       # misaligned device pointer
     assert L.aceapex_decode_all(None, None, 0, None) == binding.E_ARG
+    assert L.aceapex_decode_range(None, 0, 1, None, 0, None) == binding.E_ARG
     assert L.aceapex_decode_blocks(None, None, 0, None, 0, 0, None) == binding.E_ARG
     assert L.aceapex_seek(None, 0, None, 0, None, None, None) == binding.E_ARG
     assert L.aceapex_scratch_bytes(None, 1, 1) == 0

@@ -315,6 +315,76 @@ def test_rejects_inconsistent_tag(binding):
         assert rc == binding.E_CORRUPT and first == 1
 
 
+# ------------------------------------------------------------------ range decode
+
+def check_range(binding, dec, want, first, count, fill=0xA5):
+    """decode_range(first, count) into a guarded range-sized buffer == want's bytes; nothing outside is written."""
+    n = want.size
+    lo, hi = first * B, min(n, (first + count) * B)
+    guard = 4096
+    buf = dev_out(guard + count * B + guard, fill)
+    dec.decode_range(first, count, buf[guard:])
+    dec.check()
+    got = buf.cpu().numpy()
+    assert np.array_equal(got[guard:guard + hi - lo], want[lo:hi]), (first, count)
+    assert np.all(got[:guard] == fill) and np.all(got[guard + hi - lo:] == fill), (first, count)
+
+
+@pytest.mark.parametrize("policy", ["scheduled", "literal", "small_window"])
+def test_range_decode_samples(binding, policy):
+    """Ranges at the start, in the middle and at the ragged end of a text sample under three encoder policies: with
+    the literal policy and the small window most cross-block sources of a mid-file range lie INSIDE the range (match
+    kernel), with the scheduled window all of them lie below it (isolated chase); sub-batches smaller than the range."""
+    data = W.generate("text", 150 * B + 4321, 91)
+    params = {"scheduled": dict(min_match=8, max_depth=8, window=64, batch=8, max_level=1, raw_slack_pct=5),
+              "literal": dict(W.POLICY_LITERAL), "small_window": dict(min_match=6, max_depth=6, window=3, batch=3)}[policy]
+    c = oracle.encode(data, threads=8, **params)
+    want = oracle.decode_all(c)
+    assert np.array_equal(want, data)
+    nb = int(oracle.info(c).n_blocks)
+    with binding.Decoder(c, n_targets=64) as dec:
+        for first, count in ((0, 40), (0, nb), (1, 1), (37, 50), (100, nb - 100), (nb - 1, 1), (70, 3)):
+            check_range(binding, dec, want, first, count)
+        L = binding.lib()
+        buf = dev_out(4 * B)
+        assert L.aceapex_decode_range(dec._ctx, nb - 1, 2, buf.data_ptr(), buf.numel(), None) == binding.E_RANGE
+        assert L.aceapex_decode_range(dec._ctx, 5, 4, buf.data_ptr(), 4 * B - 1, None) == binding.E_CAPACITY
+        assert L.aceapex_decode_range(dec._ctx, 5, 0, None, 0, None) == 0
+    with binding.Decoder(c, n_slots=7, n_targets=5) as dec:          # sub-batches of 5 blocks (PAPER.md:112)
+        check_range(binding, dec, want, 60, 23)
+        check_range(binding, dec, want, 0, 23)
+    with binding.Decoder(c, n_targets=0) as dec:                     # no isolated scratch: only ranges from block 0
+        check_range(binding, dec, want, 0, 30)
+        buf = dev_out(2 * B)
+        assert binding.lib().aceapex_decode_range(dec._ctx, 3, 2, buf.data_ptr(), buf.numel(), None) == binding.E_STATE
+
+
+def test_range_decode_handmade_spanning_and_deep(binding):
+    """The handmade container (a source that spans two blocks, tags 1..11, escapes): every range of it."""
+    total, blocks = handmade_case()
+    c = container_from_tokens(total, blocks)
+    want = np.frombuffer(expand(total, blocks), np.uint8)
+    with binding.Decoder(c, n_targets=2) as dec:
+        for first in range(3):
+            for count in range(1, 4 - first):
+                check_range(binding, dec, want, first, count, fill=0x00)
+                check_range(binding, dec, want, first, count)
+
+
+def test_range_decode_text_256m_blocks_0_1000_and_mid_file(binding):
+    """SURVEY.md section 8(f)-2 / PAPER.md:104: blocks 0-1000 and a mid-file range of 1,001 blocks of configs[3]
+    into a 1,001-block buffer, bit-exact against the original bytes (= decoder #1), nothing written outside."""
+    cfg = W.CONFIGS["text_256m"]
+    data = cfg.data()
+    c = oracle.encode(data, offset_width=cfg.offset_width, threads=32, **cfg.encoder)
+    nb = int(oracle.info(c).n_blocks)
+    with binding.Decoder(c, n_targets=1024) as dec:
+        check_range(binding, dec, data, 0, 1001)
+        check_range(binding, dec, data, nb // 2, 1001)
+        check_range(binding, dec, data, nb - 1001, 1001)
+        check_range(binding, dec, data, 5000, 3000)                  # three sub-batches of 1,024 targets
+
+
 # ------------------------------------------------------------------ isolation
 
 @pytest.mark.parametrize("fill", [0x00, 0xA5])
