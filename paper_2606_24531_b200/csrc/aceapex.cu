@@ -29,6 +29,7 @@ struct aceapex_ctx {
     uint64_t launches = 0;
     int sm_count = 0;
     int match_ctas_per_sm = 0;
+    int entropy_ctas_per_sm = 0;
     int seek_ctas_per_sm = 0;
     int device = 0;
     bool prof = false;
@@ -111,7 +112,12 @@ int launch_entropy(aceapex_ctx *c, const uint64_t *list, const uint32_t *n_list,
 {
     uint32_t units = 3 * (list ? max_slots : count);
     uint32_t grid = (units + kEntropyWarps - 1) / kEntropyWarps;
-    uint32_t cap = (uint32_t)c->sm_count * 2;   // 2 CTAs of 16 warps per SM (shared memory)
+    if (c->entropy_ctas_per_sm == 0) {         // persistent warps: one wave of resident CTAs (2 of 16 warps per SM)
+        int nb = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_entropy, 32 * (int)kEntropyWarps, entropy_smem()) != cudaSuccess || nb < 1) nb = 1;
+        c->entropy_ctas_per_sm = nb;
+    }
+    uint32_t cap = (uint32_t)c->sm_count * (uint32_t)c->entropy_ctas_per_sm;
     if (grid > cap) grid = cap;
     if (grid == 0) return ACEAPEX_OK;
     {

@@ -20,7 +20,13 @@ namespace aceapex {
 constexpr uint32_t kT8Bytes = kM;
 constexpr uint32_t kSymlBytes = 256 * 8;
 constexpr uint32_t kRingBytes = 512;
-constexpr uint32_t kEntropyWarps = 16;
+// Warps per entropy CTA (each warp decodes one stream at a time with its own tables). Swept through
+// -DACEAPEX_ENTROPY_WARPS (8 or 16; PAPER.md:86-92 sweeps the threads per parser the same way).
+#ifndef ACEAPEX_ENTROPY_WARPS
+#define ACEAPEX_ENTROPY_WARPS 16
+#endif
+constexpr uint32_t kEntropyWarps = ACEAPEX_ENTROPY_WARPS;
+static_assert(kEntropyWarps == 4 || kEntropyWarps == 8 || kEntropyWarps == 16, "entropy CTA size");
 constexpr uint32_t kEntropySmem = kEntropyWarps * (kT8Bytes + kSymlBytes + kRingBytes) + kT8Bytes;   // + alignment slack
 constexpr uint32_t kRingWords = 256, kRingChunk = 64;
 
@@ -50,6 +56,17 @@ __device__ inline uint2 lds_v2(uint32_t a)
 }
 
 __device__ inline uint32_t lane_id() { return threadIdx.x & 31u; }
+
+// "Am I lane 0", read afresh every time. A leader branch written as `lane == 0` invites the compiler to thread
+// several such tests into one and to duplicate the code between them for the two outcomes: lane 0 then runs
+// its own copy of a whole stream decode beside the other 31 lanes (measured on k_entropy: 75 -> 180 us when one
+// more leader branch was added to decode_unit). An opaque read keeps every leader branch a small diamond.
+__device__ inline bool leader()
+{
+    uint32_t l;
+    asm volatile("mov.u32 %0, %%laneid;" : "=r"(l));
+    return l == 0;
+}
 
 __device__ inline uint32_t warp_excl_scan(uint32_t v, uint32_t lane, uint32_t &total)
 {
@@ -274,7 +291,8 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
     SlotHdr *hdr = reinterpret_cast<SlotHdr *>(slot + sl.o_hdr);
     const Record r = open_record(cv, blk);
     bool ok = r.ok;
-    if (write_hdr && ok && lane == 0) {
+    // (stored by every lane - same address, same value, one transaction - rather than under a leader branch)
+    if (write_hdr && ok) {
         hdr->n_seq = r.n_seq; hdr->n_lit = r.n_lit; hdr->block_len = r.block_len;
         hdr->n_extras = r.n_extras; hdr->off_nbytes = r.off_nbytes;
         hdr->extras_off = r.extras_off; hdr->tags_off = r.tags_off;
@@ -299,11 +317,11 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
         const uint32_t is_raw = s == LIT ? r.raw[LIT] : (s == LEN ? r.raw[LEN] : r.raw[OFF]);
         if (is_raw) ok = copy_raw_stream(x0, n, r.rec + wo, out, lane);
         else ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
-        if (!ok && lane == 0) raise(ctl, kStEntropy, blk);
-    } else if (lane == 0) {
+        if (!ok && leader()) raise(ctl, kStEntropy, blk);
+    } else if (leader()) {
         raise(ctl, kStRecord, blk);
     }
-    if (lane == 0) hdr->bad[s] = ok ? 0u : 1u;
+    hdr->bad[s] = ok ? 0u : 1u;
     __syncwarp();
 }
 
@@ -336,7 +354,7 @@ __global__ void __launch_bounds__(32 * kEntropyWarps) k_entropy(Container cv, Sl
     const uint32_t n_units = 3 * nb;
     for (;;) {
         uint32_t u = 0;
-        if (lane == 0) u = atomicAdd(&ctl->unit, 1u);
+        if (leader()) u = atomicAdd(&ctl->unit, 1u);
         u = __shfl_sync(0xFFFFFFFFu, u, 0);
         if (u >= n_units) break;
         // longest first: all LIT streams, then OFF, then LEN (balances the tail of the launch)
