@@ -48,7 +48,7 @@ def build(force: bool = False) -> str:
 class EncParams(C.Structure):
     _fields_ = [(n, C.c_uint32) for n in
                 ("min_match", "chain_depth", "max_depth", "window", "max_level", "offset_width", "threads", "batch",
-                 "raw_slack_pct")]
+                 "raw_slack_pct", "max_fanout", "long_hash", "long_chain")]
 
 
 class EncStats(C.Structure):
@@ -61,7 +61,8 @@ class EncStats(C.Structure):
 class Info(C.Structure):
     _fields_ = [("total_len", C.c_uint64), ("n_blocks", C.c_uint64), ("payload_off", C.c_uint64),
                 ("container_bytes", C.c_uint64), ("offset_width", C.c_uint32), ("max_depth", C.c_uint32),
-                ("window", C.c_uint32), ("max_level", C.c_uint32), ("min_match_policy", C.c_uint32)]
+                ("window", C.c_uint32), ("max_level", C.c_uint32), ("min_match_policy", C.c_uint32),
+                ("max_fanout", C.c_uint32)]
 
 
 class BlockHdr(C.Structure):

@@ -74,6 +74,11 @@ typedef struct {
                               RAW when n_sym * 100 <= (tbl_bytes + 2 * n_words) * (100 + raw_slack_pct), i.e.
                               when rANS saves less than that margin. Default 0: RAW only where rANS does not
                               shrink the stream. 0xFFFFFFFF: never RAW. */
+    uint32_t max_fanout;   /* F: the matches of a block read from at most F distinct earlier blocks (seek-aware
+                              policy; header promise, FORMAT.md section 1); 0 = unbounded */
+    uint32_t long_hash;    /* 0, or 9..16: bytes keyed by a second global hash table that is probed first
+                              (SURVEY.md reading A14: 12) */
+    uint32_t long_chain;   /* candidates tried on the long-hash chain (default 16) */
 } ora_enc_params;
 
 typedef struct {
@@ -92,7 +97,7 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *p, uint8_t *ou
 
 typedef struct {
     uint64_t total_len, n_blocks, payload_off, container_bytes;
-    uint32_t offset_width, max_depth, window, max_level, min_match_policy;
+    uint32_t offset_width, max_depth, window, max_level, min_match_policy, max_fanout;
 } ora_info;
 
 int ora_info_get(const uint8_t *c, size_t clen, ora_info *out);

@@ -31,7 +31,8 @@ int ora_container_open(const uint8_t *c, size_t clen, ora_container *out)
     I->max_depth = rd32(c + 32);
     I->window = rd32(c + 36);
     I->max_level = rd32(c + 40);
-    I->min_match_policy = rd32(c + 44);
+    I->min_match_policy = rd32(c + 44) & 0xFFFFu;
+    I->max_fanout = rd32(c + 44) >> 16;
     uint64_t index_off = rd64(c + 48);
     I->payload_off = rd64(c + 56);
     if (I->n_blocks != (I->total_len + ORA_B - 1) / ORA_B) return ORA_E_FORMAT;
@@ -481,6 +482,7 @@ int ora_validate(const uint8_t *c, size_t clen, ora_validate_report *rep)
         }
         for (uint32_t i = 0; i < n_touched; i++) seen[touched[i] >> 6] &= ~((uint64_t)1 << (touched[i] & 63));
         if (n_src_blocks > R.max_src_blocks_per_block) R.max_src_blocks_per_block = n_src_blocks;
+        if (k.info.max_fanout && n_src_blocks > k.info.max_fanout) promise_broken = 1;
         sum_src_blocks += n_src_blocks;
     }
     if (rc == ORA_OK) {

@@ -18,6 +18,13 @@
  *   j+l <= end of eligible region (R > 0, global candidates), every source byte of copy depth
  *   < D (D > 0) and, inside the block, of tag < max_level. The longest wins, the first found
  *   among equals; it is accepted if l >= T. Otherwise in[i] is a literal.
+ *   long_hash > 0 (SURVEY.md reading A14: "4-byte hash + optional 12-byte long hash; chain depth 32
+ *   (+16 long)"): a second global table keyed on long_hash bytes is probed first, up to long_chain
+ *   candidates, newest first, under the same limits; then the chains above.
+ *   max_fanout F > 0 (seek-aware policy; a seek needs every block
+ *   a block copies from): the matches of one block read from at most F distinct earlier blocks. A global
+ *   candidate whose first source block is neither used yet nor affordable is skipped; one that runs on
+ *   into a second block that is neither is cut at the block boundary.
  */
 #include "container.h"
 
@@ -52,6 +59,8 @@ typedef struct {
     uint8_t off_sym[8 * ORA_MAX_SEQ];
     uint16_t extras[2 * ORA_MAX_SEQ];
     uint16_t words[3][8 * ORA_MAX_SEQ];
+    uint64_t *fan_bits;    /* max_fanout: bitmap over blocks, the source blocks this block uses */
+    uint32_t fan_list[2 * ORA_MAX_SEQ], fan_n;
 } enc_scratch;
 
 typedef struct {
@@ -62,6 +71,9 @@ typedef struct {
     uint32_t *head;  /* position+1 of the newest inserted position per hash, 0 = empty */
     uint32_t *prev;  /* position+1 of the previous position with the same hash */
     uint8_t *depth;  /* copy-hop depth of every parsed byte (saturating at 255) */
+    uint32_t long_bits;
+    uint32_t *head2; /* long hash: same scheme, keyed on p.long_hash bytes */
+    uint32_t *prev2;
 } enc_ctx;
 
 void ora_enc_params_default(ora_enc_params *p)
@@ -75,6 +87,9 @@ void ora_enc_params_default(ora_enc_params *p)
     p->threads = 1;
     p->batch = 64;
     p->raw_slack_pct = 0;
+    p->max_fanout = 0;
+    p->long_hash = 0;
+    p->long_chain = 16;
 }
 
 size_t ora_encode_bound(size_t n)
@@ -92,6 +107,15 @@ static inline uint32_t hash_at(const enc_ctx *e, size_t i)
     return (uint32_t)((v * 0x9E3779B97F4A7C15ull) >> (64 - e->hash_bits));
 }
 
+static inline uint32_t long_hash_at(const enc_ctx *e, size_t i)
+{
+    uint64_t a = 0, b = 0;
+    const uint32_t nb = e->p.long_hash;          /* 9..16 */
+    memcpy(&a, e->in + i, 8);
+    memcpy(&b, e->in + i + 8, nb - 8);
+    return (uint32_t)(((a * 0x9E3779B97F4A7C15ull) ^ (b * 0xC2B2AE3D27D4EB4Full)) * 0x9E3779B97F4A7C15ull >> (64 - e->long_bits));
+}
+
 static void global_insert(enc_ctx *e, size_t from, size_t to)
 {
     for (size_t p = from; p < to; p++) {
@@ -100,7 +124,32 @@ static void global_insert(enc_ctx *e, size_t from, size_t to)
         uint32_t h = hash_at(e, p);
         e->prev[p] = e->head[h];
         e->head[h] = (uint32_t)p + 1;
+        if (e->head2 && p + e->p.long_hash <= e->n) {
+            uint32_t h2 = long_hash_at(e, p);
+            e->prev2[p] = e->head2[h2];
+            e->head2[h2] = (uint32_t)p + 1;
+        }
     }
+}
+
+/* max_fanout: how far a global candidate at j may run, given the source blocks the block already uses */
+static inline int fan_has(const enc_scratch *s, uint64_t blk) { return (int)(s->fan_bits[blk >> 6] >> (blk & 63) & 1); }
+static inline uint32_t fan_limit(const enc_ctx *e, const enc_scratch *s, size_t j, uint32_t maxlen)
+{
+    const uint32_t F = e->p.max_fanout;
+    if (!F) return maxlen;
+    const uint64_t b0 = j >> ORA_BLOG;
+    uint32_t room = F - s->fan_n;
+    if (!fan_has(s, b0)) { if (!room) return 0; room--; }
+    const size_t to_end = ((size_t)(b0 + 1) << ORA_BLOG) - j;      /* bytes left in block b0 */
+    if (maxlen > to_end && !fan_has(s, b0 + 1) && !room) maxlen = (uint32_t)to_end;
+    return maxlen;
+}
+static inline void fan_add(enc_scratch *s, uint64_t blk)
+{
+    if (fan_has(s, blk)) return;
+    s->fan_bits[blk >> 6] |= (uint64_t)1 << (blk & 63);
+    s->fan_list[s->fan_n++] = (uint32_t)blk;
 }
 
 /* candidate j for position i: common prefix under all limits of the definition above */
@@ -131,6 +180,7 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
     size_t lit_start = B0, i = B0;
     memset(s->lhead, 0xFF, sizeof s->lhead);
     memset(s->level, 0, sizeof s->level);
+    s->fan_n = 0;
 
     while (i < B1) {
         uint32_t best = 0;
@@ -149,6 +199,19 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
                 uint32_t l = try_candidate(e, s->level, B0, i, j, maxlen, best);
                 if (l > best) { best = l; best_src = j; }
             }
+            /* the long-hash global chain, newest first */
+            if (e->head2 && i + e->p.long_hash <= e->n) {
+                uint32_t g = e->head2[long_hash_at(e, i)];
+                for (uint32_t steps = 0; g != 0 && steps < e->p.long_chain; steps++, g = e->prev2[g - 1]) {
+                    size_t j = g - 1;
+                    uint32_t maxlen = remaining;
+                    if (i - j < maxlen) maxlen = (uint32_t)(i - j);
+                    if (e->p.window && elig_end - j < maxlen) maxlen = (uint32_t)(elig_end - j);
+                    maxlen = fan_limit(e, s, j, maxlen);
+                    uint32_t l = try_candidate(e, s->level, B0, i, j, maxlen, best);
+                    if (l > best) { best = l; best_src = j; }
+                }
+            }
             /* the global chain, newest first */
             uint32_t g = e->head[h];
             for (uint32_t steps = 0; g != 0 && steps < chain; steps++, g = e->prev[g - 1]) {
@@ -156,6 +219,7 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
                 uint32_t maxlen = remaining;
                 if (i - j < maxlen) maxlen = (uint32_t)(i - j);
                 if (e->p.window && elig_end - j < maxlen) maxlen = (uint32_t)(elig_end - j);
+                maxlen = fan_limit(e, s, j, maxlen);
                 uint32_t l = try_candidate(e, s->level, B0, i, j, maxlen, best);
                 if (l > best) { best = l; best_src = j; }
             }
@@ -174,6 +238,11 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
             }
             d = d + 1 > 255 ? 255 : d + 1;
             q->tag = (uint8_t)lv;
+            if (e->p.max_fanout && best_src < B0) {
+                fan_add(s, best_src >> ORA_BLOG);
+                const uint64_t lastb = (best_src + best - 1) >> ORA_BLOG;
+                if (lastb < b) fan_add(s, lastb);
+            }
             if (d > st->max_depth_seen) st->max_depth_seen = d;
             if (lv > st->max_level_seen) st->max_level_seen = lv;
             st->match_bytes += best;
@@ -199,6 +268,7 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
             i++;
         }
     }
+    for (uint32_t k = 0; k < s->fan_n; k++) s->fan_bits[s->fan_list[k] >> 6] = 0;
     memcpy(s->lit + n_lit, in + lit_start, B1 - lit_start); /* trailing literals */
     n_lit += (uint32_t)(B1 - lit_start);
     *n_seq_out = n_seq;
@@ -311,6 +381,8 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *pp, uint8_t *o
     if (n >= 0xFFFFFFF0ull) return ORA_E_ARG;          /* oracle limit (u32 chains), not a format limit */
     if (e.p.offset_width == 4 && n > 0xFFFFFFFFull) return ORA_E_ARG;
     if (e.p.max_depth > 254) return ORA_E_ARG;
+    if (e.p.max_fanout > 0xFFFF || e.p.min_match > 0xFFFF) return ORA_E_ARG;
+    if (e.p.long_hash && (e.p.long_hash < 9 || e.p.long_hash > 16 || e.p.long_chain < 1)) return ORA_E_ARG;
     if (e.p.threads < 1) e.p.threads = 1;
     if (e.p.batch < 1) e.p.batch = 1;
     e.hash_bytes = e.p.min_match < 8 ? e.p.min_match : 8;
@@ -327,6 +399,17 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *pp, uint8_t *o
     e.prev = (uint32_t *)malloc(sizeof(uint32_t) * (n ? n : 1));
     e.depth = (uint8_t *)calloc(n ? n : 1, 1);
     if (!blocks || !scr || !e.head || !e.prev || !e.depth) { rc = ORA_E_NOMEM; goto done; }
+    for (uint32_t t = 0; t < e.p.threads; t++) scr[t].fan_bits = NULL;
+    for (uint32_t t = 0; t < e.p.threads; t++) {
+        scr[t].fan_bits = (uint64_t *)calloc((size_t)(nb / 64 + 2), 8);
+        if (!scr[t].fan_bits) { rc = ORA_E_NOMEM; goto done; }
+    }
+    if (e.p.long_hash) {
+        e.long_bits = e.hash_bits;
+        e.head2 = (uint32_t *)calloc((size_t)1 << e.long_bits, sizeof(uint32_t));
+        e.prev2 = (uint32_t *)malloc(sizeof(uint32_t) * (n ? n : 1));
+        if (!e.head2 || !e.prev2) { rc = ORA_E_NOMEM; goto done; }
+    }
 
     size_t inserted = 0;
     for (uint64_t s = 0; s < nb && rc == ORA_OK; s += P) {
@@ -391,13 +474,14 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *pp, uint8_t *o
         }
         wr64(rec_off + nb * 8, o);
         wr32(out + 32, e.p.max_depth); wr32(out + 36, e.p.window);
-        wr32(out + 40, S.max_level_seen); wr32(out + 44, e.p.min_match);
+        wr32(out + 40, S.max_level_seen); wr32(out + 44, e.p.min_match | e.p.max_fanout << 16);
         wr64(out + 48, ORA_HDR_BYTES); wr64(out + 56, payload_off);
         *out_len = (size_t)(payload_off + payload);
         if (stats) *stats = S;
     }
 done:
     if (blocks) for (uint64_t b = 0; b < nb; b++) free(blocks[b].rec);
-    free(blocks); free(scr); free(e.head); free(e.prev); free(e.depth);
+    if (scr) for (uint32_t t = 0; t < e.p.threads; t++) free(scr[t].fan_bits);
+    free(blocks); free(scr); free(e.head); free(e.prev); free(e.depth); free(e.head2); free(e.prev2);
     return rc;
 }

@@ -75,15 +75,22 @@ class Config:
 # >= 4 bytes, no scheduling promises); `scheduled` is the policy the large configs run with
 # (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks, in-block copy level 1,
 # and a stream is stored RAW when rANS would save less than 5 % of it (selective entropy).
+# `seek_aware` (a seek needs the blocks a block copies from) bounds what one
+# isolated block costs: copy depth <= 4 hops and at most 32 distinct source blocks per block, both header promises
+# the validator checks. `long` adds the 12-byte long hash of SURVEY.md reading A14 (genome: the "match-dominated"
+# config; 3x the encode time, so the other configs keep the short hash).
 POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
 POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1, raw_slack_pct=5)
+POLICY_SCHEDULED_LONG = dict(POLICY_SCHEDULED, long_hash=12, long_chain=16)
+POLICY_SEEK_AWARE = dict(POLICY_SCHEDULED, max_depth=4, max_fanout=32)
+POLICIES = {"literal": POLICY_LITERAL, "scheduled": POLICY_SCHEDULED, "seek_aware": POLICY_SEEK_AWARE}
 
 CONFIGS = {
     "markov_1m": Config("markov_1m", "markov", 1 * MIB, SEED_BASE + 1, 4, POLICY_LITERAL,
                         "smoke config (BASELINE.json configs[0])"),
     "fastq_64m": Config("fastq_64m", "fastq", 64 * MIB, SEED_BASE + 2, 4, POLICY_SCHEDULED,
                         "clean (real FASTQ NA12878), PAPER.md:65"),
-    "genome_256m": Config("genome_256m", "genome", 256 * MIB, SEED_BASE + 3, 8, POLICY_SCHEDULED,
+    "genome_256m": Config("genome_256m", "genome", 256 * MIB, SEED_BASE + 3, 8, POLICY_SCHEDULED_LONG,
                           "repeat (repetitive genome), PAPER.md:66"),
     "text_256m": Config("text_256m", "text", 256 * MIB, SEED_BASE + 4, 4, POLICY_SCHEDULED,
                         "enwik9 (English text), PAPER.md:67"),

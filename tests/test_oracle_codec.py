@@ -316,3 +316,46 @@ def test_rejects_inconsistent_raw_streams():
     pos = oracle.info(c).payload_off + 32 + 3                             # first section after the header = words[LIT]
     bad = c.copy(); assert bad[pos] == 0; bad[pos] = 1
     rejected(bad)
+
+
+def test_seek_aware_policy_bounds_fanout_and_depth_and_validator_checks_them():
+    """SURVEY.md section 8f rank 4 (a seek needs every block a block copies from): max_fanout F and
+    max_depth D are header promises; the validator recomputes both from the tokens alone."""
+    cfg = W.CONFIGS["text_256m"]
+    data = cfg.data(3 * 1024 * 1024)
+    base = dict(W.POLICY_SCHEDULED, window=16, batch=8)                # a window the 192-block sample can use
+    c0 = oracle.encode(data, offset_width=4, **base)
+    r0 = oracle.validate(c0)
+    assert r0.max_src_blocks_per_block > 12                            # the unbounded policy really fans out
+    for F, D in ((12, 8), (4, 2)):
+        c = oracle.encode(data, offset_width=4, **dict(base, max_fanout=F, max_depth=D))
+        assert np.array_equal(oracle.decode_all(c), data)
+        i = oracle.info(c)
+        assert (i.max_fanout, i.max_depth, i.min_match_policy) == (F, D, 8)
+        r = oracle.validate(c)                                         # raises if a promise is broken
+        assert r.max_src_blocks_per_block <= F and r.max_depth_seen <= D
+        assert c.size >= c0.size                                       # a bound can only cost ratio
+    # a container that promises less than it keeps: same tokens, header fan-out lowered to 2
+    bad = c0.copy()
+    bad[46:48] = np.frombuffer(np.uint16(2).tobytes(), np.uint8)
+    assert np.array_equal(oracle.decode_all(bad), data)                # decoding never depends on a promise
+    with pytest.raises(oracle.OracleError) as e:
+        oracle.validate(bad)
+    assert e.value.code == -7
+
+
+def test_long_hash_finds_longer_matches_and_round_trips():
+    """SURVEY.md reading A14: optional 12-byte long hash, probed first. Same format, same decoders."""
+    cfg = W.CONFIGS["genome_256m"]
+    data = cfg.data(2 * 1024 * 1024)
+    short = dict(W.POLICY_SCHEDULED, window=16, batch=8)
+    c_s, st_s = oracle.encode(data, return_stats=True, offset_width=8, **short)
+    c_l, st_l = oracle.encode(data, return_stats=True, offset_width=8, threads=3, **dict(short, long_hash=12))
+    c_l1 = oracle.encode(data, offset_width=8, threads=1, **dict(short, long_hash=12))
+    assert np.array_equal(c_l, c_l1)                                   # independent of the thread count
+    assert np.array_equal(oracle.decode_all(c_l), data)
+    oracle.validate(c_l)
+    assert st_l.match_bytes / st_l.n_seq > st_s.match_bytes / st_s.n_seq and c_l.size < c_s.size
+    with oracle.Isolated(c_l) as iso:
+        for b in (0, 57, 127):
+            assert np.array_equal(iso.decode(b), data[b * 16384:(b + 1) * 16384])
