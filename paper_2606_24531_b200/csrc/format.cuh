@@ -125,8 +125,8 @@ struct Control {
     uint32_t unit, unit_exit;       // entropy kernel: (block, stream) unit hand-out
     uint32_t rsv1;
     uint32_t max_n_seq;             // open-time scan result
-    // fused isolated decode (seek.cuh): grid barrier and counters, double-buffered by round / hop parity
-    uint32_t bar_count, bar_gen;
+    // fused isolated decode (seek.cuh): counters, double-buffered by round / hop parity
+    uint32_t rsv3[2];
     uint32_t round_n_list[2];       // distinct blocks claimed so far in the round (by round parity)
     uint32_t rsv2[3];
     unsigned long long hop_pending[2];   // bytes still chasing after the hop (by hop parity)
