@@ -54,7 +54,10 @@ def lib():
     global _lib
     with _lock:
         if _lib is None:
-            path = _build.build()
+            # ACEAPEX_LIB: a variant built by build.build_variant (granularity sweeps); otherwise the in-tree library
+            path = os.environ.get("ACEAPEX_LIB") or _build.build()
+            if not os.path.exists(path):
+                raise RuntimeError(f"{path}: CUDA library not found (there is no CPU fallback)")
             L = C.CDLL(path)
             vp, sz, u64, u32 = C.c_void_p, C.c_size_t, C.c_uint64, C.c_uint32
             L.aceapex_version.restype = C.c_int

@@ -54,5 +54,22 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return SO
 
 
+def build_variant(name: str, defines: dict, verbose: bool = False) -> str:
+    """Compile the library with extra -D macros (the granularity knobs of PAPER.md:86-92 in this design:
+    ACEAPEX_MATCH_THREADS, ACEAPEX_ENTROPY_WARPS) into build/libaceapex_<name>.so; `bench.py --sweep` loads
+    such a variant through the ACEAPEX_LIB environment variable."""
+    out_dir = os.path.join(_DIR, "build")
+    os.makedirs(out_dir, exist_ok=True)
+    so = os.path.join(out_dir, f"libaceapex_{name}.so")
+    flags = [f"-D{k}={v}" for k, v in sorted(defines.items())]
+    cmd = [nvcc()] + NVCC_FLAGS + flags + (["-Xptxas", "-v"] if verbose else []) + ["-o", so] + \
+          [os.path.join(CSRC, s) for s in SOURCES]
+    r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed")
+    return so
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
