@@ -48,7 +48,7 @@ def build(force: bool = False) -> str:
 class EncParams(C.Structure):
     _fields_ = [(n, C.c_uint32) for n in
                 ("min_match", "chain_depth", "max_depth", "window", "max_level", "offset_width", "threads", "batch",
-                 "raw_slack_pct", "max_fanout", "long_hash", "long_chain")]
+                 "raw_slack_pct", "max_fanout", "long_hash", "long_chain", "max_seq")]
 
 
 class EncStats(C.Structure):

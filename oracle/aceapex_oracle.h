@@ -79,6 +79,8 @@ typedef struct {
     uint32_t long_hash;    /* 0, or 9..16: bytes keyed by a second global hash table that is probed first
                               (SURVEY.md reading A14: 12) */
     uint32_t long_chain;   /* candidates tried on the long-hash chain (default 16) */
+    uint32_t max_seq;      /* at most this many sequences per block, the rest of a block is literals; 0 = the format
+                              limit (4096) */
 } ora_enc_params;
 
 typedef struct {

@@ -25,6 +25,8 @@
  *   a block copies from): the matches of one block read from at most F distinct earlier blocks. A global
  *   candidate whose first source block is neither used yet nor affordable is skipped; one that runs on
  *   into a second block that is neither is cut at the block boundary.
+ *   max_seq > 0: a block holds at most max_seq sequences; once it has that many, the rest of the block is
+ *   literals (a decoder sizes its per-block tables for the densest block of a container).
  */
 #include "container.h"
 
@@ -90,6 +92,7 @@ void ora_enc_params_default(ora_enc_params *p)
     p->max_fanout = 0;
     p->long_hash = 0;
     p->long_chain = 16;
+    p->max_seq = 0;
 }
 
 size_t ora_encode_bound(size_t n)
@@ -176,6 +179,7 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
     const size_t B1 = (B0 + ORA_B < e->n) ? B0 + ORA_B : e->n;
     const uint32_t T = e->p.min_match, chain = e->p.chain_depth, D = e->p.max_depth, L = e->p.max_level;
     const uint32_t lmask = (1u << LOCAL_HASH_BITS) - 1;
+    const uint32_t max_seq = e->p.max_seq && e->p.max_seq < ORA_MAX_SEQ ? e->p.max_seq : ORA_MAX_SEQ;
     uint32_t n_seq = 0, n_lit = 0;
     size_t lit_start = B0, i = B0;
     memset(s->lhead, 0xFF, sizeof s->lhead);
@@ -189,7 +193,7 @@ static void parse_block(enc_ctx *e, uint64_t b, size_t elig_end, enc_scratch *s,
         const int can_hash = i + e->hash_bytes <= e->n;
         uint32_t h = 0;
         if (can_hash) h = hash_at(e, i);
-        if (can_hash && remaining >= T) {
+        if (can_hash && remaining >= T && n_seq < max_seq) {
             /* the block's own chain, newest first */
             uint32_t cand = s->lhead[h & lmask];
             for (uint32_t steps = 0; cand != NONE16 && steps < chain; steps++, cand = s->lprev[cand]) {

@@ -80,8 +80,12 @@ class Config:
 # the validator checks. `long` adds the 12-byte long hash of SURVEY.md reading A14 (genome: the "match-dominated"
 # config; 3x the encode time, so the other configs keep the short hash).
 POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
-POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1, raw_slack_pct=5)
-POLICY_SCHEDULED_LONG = dict(POLICY_SCHEDULED, long_hash=12, long_chain=16)
+# `max_seq`: at most that many sequences per block (the rest of a dense block stays literal). The match kernel sizes
+# every CTA's tables for the densest block of a container; 1536 (4-byte offsets) resp. 1344 (8-byte) keeps four CTAs
+# resident per SM, and touches about one block in a hundred.
+POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1, raw_slack_pct=5,
+                        max_seq=1536)
+POLICY_SCHEDULED_LONG = dict(POLICY_SCHEDULED, long_hash=12, long_chain=16, max_seq=1344)
 POLICY_SEEK_AWARE = dict(POLICY_SCHEDULED, max_depth=4, max_fanout=32)
 POLICIES = {"literal": POLICY_LITERAL, "scheduled": POLICY_SCHEDULED, "seek_aware": POLICY_SEEK_AWARE}
 

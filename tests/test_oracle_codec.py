@@ -359,3 +359,16 @@ def test_long_hash_finds_longer_matches_and_round_trips():
     with oracle.Isolated(c_l) as iso:
         for b in (0, 57, 127):
             assert np.array_equal(iso.decode(b), data[b * 16384:(b + 1) * 16384])
+
+
+def test_max_seq_caps_sequences_per_block():
+    """Encoder knob max_seq: a block never holds more sequences; what follows in the block is literal."""
+    data = W.generate("text", 1 << 20, 99)
+    base = dict(min_match=4, chain_depth=32)
+    c0, st0 = oracle.encode(data, return_stats=True, **base)
+    c1, st1 = oracle.encode(data, return_stats=True, max_seq=300, **base)
+    assert np.array_equal(oracle.decode_all(c1), data)
+    oracle.validate(c1)
+    n0 = [oracle.decode_streams(c0, b)[0].n_seq for b in range(64)]
+    n1 = [oracle.decode_streams(c1, b)[0].n_seq for b in range(64)]
+    assert max(n0) > 300 and max(n1) == 300 and st1.n_seq < st0.n_seq and c1.size > c0.size
