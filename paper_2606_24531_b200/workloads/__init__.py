@@ -76,8 +76,9 @@ class Config:
 # (reading A15): threshold 8, copy depth <= 8, window of 1024 blocks, in-block copy level 1,
 # and a stream is stored RAW when rANS would save less than 5 % of it (selective entropy).
 # `seek_aware` (a seek needs the blocks a block copies from) bounds what one
-# isolated block costs: copy depth <= 4 hops and at most 32 distinct source blocks per block, both header promises
-# the validator checks. `long` adds the 12-byte long hash of SURVEY.md reading A14 (genome: the "match-dominated"
+# isolated block costs: copy depth <= 3 hops and at most 128 distinct source blocks per block, both header promises
+# the validator checks (a single seek's latency follows the hops; the fan-out bound mostly helps batches, and 32
+# instead of 128 would cost the genome profile half its ratio: BASELINE.md). `long` adds the 12-byte long hash of SURVEY.md reading A14 (genome: the "match-dominated"
 # config; 3x the encode time, so the other configs keep the short hash).
 POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
 # `max_seq`: at most that many sequences per block (the rest of a dense block stays literal). The match kernel sizes
@@ -86,7 +87,7 @@ POLICY_LITERAL = dict(min_match=4, chain_depth=32, max_depth=0, window=0)
 POLICY_SCHEDULED = dict(min_match=8, chain_depth=32, max_depth=8, window=1024, batch=64, max_level=1, raw_slack_pct=5,
                         max_seq=1536)
 POLICY_SCHEDULED_LONG = dict(POLICY_SCHEDULED, long_hash=12, long_chain=16, max_seq=1344)
-POLICY_SEEK_AWARE = dict(POLICY_SCHEDULED, max_depth=4, max_fanout=32)
+POLICY_SEEK_AWARE = dict(POLICY_SCHEDULED, max_depth=3, max_fanout=128)
 POLICIES = {"literal": POLICY_LITERAL, "scheduled": POLICY_SCHEDULED, "seek_aware": POLICY_SEEK_AWARE}
 
 CONFIGS = {
