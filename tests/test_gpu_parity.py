@@ -81,13 +81,16 @@ SAMPLES = [("fastq_64m", 6 << 20), ("genome_256m", 6 << 20), ("text_256m", 6 << 
 
 
 @pytest.mark.parametrize("name,nbytes", SAMPLES)
-@pytest.mark.parametrize("policy", ["scheduled", "literal"])
+@pytest.mark.parametrize("policy", ["scheduled", "literal", "seek_aware"])
 def test_profile_samples_bit_exact(binding, name, nbytes, policy):
-    """Several hundred blocks of each profile, ragged tail, under both encoder policies."""
+    """Several hundred blocks of each profile, ragged tail, under the three encoder policies (seek_aware: the
+    config's own policy with the copy-depth and fan-out bounds of SURVEY.md section 8f rank 4 and a low max_seq)."""
     cfg = W.CONFIGS[name]
     nbytes += 12345                                              # ragged last block
     data = cfg.data(nbytes)
-    params = dict(cfg.encoder) if policy == "scheduled" else dict(W.POLICY_LITERAL)
+    params = dict(cfg.encoder) if policy != "literal" else dict(W.POLICY_LITERAL)
+    if policy == "seek_aware":
+        params.update(max_depth=W.POLICY_SEEK_AWARE["max_depth"], max_fanout=6, max_seq=700)
     if params.get("window"):
         params.update(window=24, batch=8)                        # scaled so that cross-block matches exist
     c = oracle.encode(data, offset_width=cfg.offset_width, threads=8, **params)
