@@ -16,13 +16,19 @@ import threading
 import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_DIR, "libaceapex_oracle.so")
+# Block size: 16 KiB (block_log2 14). ACEAPEX_BLOCK_LOG2=12..15 selects a variant of the oracle compiled
+# with -DORA_BLOG for the block-size sweep (`bench.py --sweep`).
+BLOG = int(os.environ.get("ACEAPEX_BLOCK_LOG2", "14"))
+if not 12 <= BLOG <= 15:
+    raise ValueError("ACEAPEX_BLOCK_LOG2 must be 12..15")
+_SO = os.path.join(_DIR, "libaceapex_oracle.so" if BLOG == 14 else f"libaceapex_oracle_b{BLOG}.so")
 _SRC = ["rans.c", "decoder.c", "encoder.c"]
 _HDR = ["aceapex_oracle.h", "container.h"]
 _lock = threading.Lock()
 _lib = None
 
-B = 16384
+B = 1 << BLOG
+MAX_SEQ = B // 4
 LIT, LEN, OFF = 0, 1, 2
 
 
@@ -39,7 +45,7 @@ def build(force: bool = False) -> str:
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(d) for d in deps):
         return _SO
     tmp = _SO + f".tmp{os.getpid()}"
-    cmd = ["gcc", "-std=c11", "-O2", "-g", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp] + srcs
+    cmd = ["gcc", "-std=c11", "-O2", "-g", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", f"-DORA_BLOG={BLOG}", "-o", tmp] + srcs
     subprocess.run(cmd, check=True, cwd=_DIR)
     os.replace(tmp, _SO)
     return _SO
@@ -100,6 +106,9 @@ def lib():
             L.ora_iso_close.argtypes = [vp]; L.ora_iso_close.restype = None
             L.ora_validate.argtypes = [u8p, sz, C.POINTER(ValidateReport)]
             L.ora_strerror.argtypes = [C.c_int]; L.ora_strerror.restype = C.c_char_p
+            L.ora_block_log2.restype = C.c_int
+            if L.ora_block_log2() != BLOG:
+                raise RuntimeError(f"{_SO}: compiled for block_log2 {L.ora_block_log2()}, wanted {BLOG}")
             _lib = L
     return _lib
 
@@ -208,8 +217,8 @@ def decode_streams(container, block: int):
     """Entropy-decode one block: (hdr, lit, len, off, extras, tags)."""
     c = _bytes_arr(container)
     h = BlockHdr()
-    lit = np.zeros(B, np.uint8); ln = np.zeros(8192, np.uint8); off = np.zeros(32768, np.uint8)
-    ex = np.zeros(8192, np.uint16); tags = np.zeros(4096, np.uint8)
+    lit = np.zeros(B, np.uint8); ln = np.zeros(2 * MAX_SEQ, np.uint8); off = np.zeros(8 * MAX_SEQ, np.uint8)
+    ex = np.zeros(2 * MAX_SEQ, np.uint16); tags = np.zeros(MAX_SEQ, np.uint8)
     _check(lib().ora_decode_streams(_ptr(c), c.size, block, C.byref(h), _ptr(lit), _ptr(ln), _ptr(off), _ptr(ex), _ptr(tags)),
            "decode_streams")
     return (h, lit[: h.n_sym[LIT]].copy(), ln[: h.n_sym[LEN]].copy(), off[: h.n_sym[OFF]].copy(),
@@ -220,8 +229,8 @@ def decode_tokens(container, block: int):
     """Parsed tokens of one block: (lit_len, match_len, src, tags)."""
     c = _bytes_arr(container)
     n = C.c_uint32(0)
-    ll = np.zeros(4096, np.uint32); ml = np.zeros(4096, np.uint32); src = np.zeros(4096, np.uint64)
-    tags = np.zeros(4096, np.uint8)
+    ll = np.zeros(MAX_SEQ, np.uint32); ml = np.zeros(MAX_SEQ, np.uint32); src = np.zeros(MAX_SEQ, np.uint64)
+    tags = np.zeros(MAX_SEQ, np.uint8)
     _check(lib().ora_decode_tokens(_ptr(c), c.size, block, C.byref(n), _ptr(ll), _ptr(ml), _ptr(src), _ptr(tags)),
            "decode_tokens")
     k = n.value

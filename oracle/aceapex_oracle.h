@@ -90,6 +90,9 @@ typedef struct {
     uint64_t n_raw[3];     /* streams stored RAW, per stream id */
 } ora_enc_stats;
 
+/* the block_log2 this library was compiled for (14 unless built with -DORA_BLOG) */
+int ora_block_log2(void);
+
 void ora_enc_params_default(ora_enc_params *p);
 size_t ora_encode_bound(size_t n);
 int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *p, uint8_t *out, size_t cap,

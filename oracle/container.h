@@ -6,9 +6,17 @@
 #include "aceapex_oracle.h"
 #include <string.h>
 
-#define ORA_B 16384u
+/* FORMAT.md section 1: block_log2. 14 (16 KiB) unless the library is built with -DORA_BLOG=12..15 for the
+ * block-size sweep ("block size ... governs how many independent parsers the format exposes").
+ * 16 would need more than the record header's 16-bit n_lit field. */
+#ifndef ORA_BLOG
 #define ORA_BLOG 14
-#define ORA_MAX_SEQ 4096u
+#endif
+#if ORA_BLOG < 12 || ORA_BLOG > 15
+#error "ORA_BLOG must be 12..15"
+#endif
+#define ORA_B (1u << ORA_BLOG)
+#define ORA_MAX_SEQ (ORA_B / 4u)          /* a sequence is at least 4 bytes long */
 #define ORA_HDR_BYTES 64u
 #define ORA_REC_HDR_BYTES 32u
 

@@ -78,6 +78,8 @@ typedef struct {
     uint32_t *prev2;
 } enc_ctx;
 
+int ora_block_log2(void) { return ORA_BLOG; }
+
 void ora_enc_params_default(ora_enc_params *p)
 {
     p->min_match = 4;

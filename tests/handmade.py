@@ -9,13 +9,17 @@ oracle (`oracle.rans_encode`, itself pinned by tests/test_oracle_rans.py).
 """
 from __future__ import annotations
 
+import os
 import struct
 
 import numpy as np
 
 import oracle
 
-B = 16384
+# Block size: 16 KiB unless ACEAPEX_BLOCK_LOG2 selects another one (block-size sweep: the oracle pins are
+# re-run against the variant, tests/test_oracle_blocksize.py).
+BLOG = int(os.environ.get("ACEAPEX_BLOCK_LOG2", "14"))
+B = 1 << BLOG
 
 
 def pad16(n):
@@ -121,7 +125,7 @@ def build_container(total_len, records, off_width=4, max_depth=0, window=0, max_
     assert nb == len(records)
     index_bytes = (nb + 1) * 8 + nb * 3 * 32 * 4
     payload_off = pad16(64 + index_bytes)
-    hdr = magic + struct.pack("<IBBBB", version, 14, off_width, 32, 12)
+    hdr = magic + struct.pack("<IBBBB", version, BLOG, off_width, 32, 12)
     hdr += struct.pack("<QQ", total_len, nb)
     hdr += struct.pack("<IIII", max_depth, window, max_level, min_match)
     hdr += struct.pack("<QQ", 64, payload_off)

@@ -12,16 +12,16 @@ import pytest
 import oracle
 from paper_2606_24531_b200 import workloads as W
 
-from handmade import B, build_container, build_record, container_from_tokens, expand
+from handmade import B, BLOG, build_container, build_record, container_from_tokens, expand
 
 
 def handmade_case():
     """3 blocks: doubling matches with length escapes and tags 1..11; a source spanning two blocks;
     a min-length match; a literal-length escape; a block with no literals at all."""
     total = 2 * B + 100
-    seqs0 = [(8, 8, 0)] + [(0, 1 << k, 0) for k in range(4, 14)]
+    seqs0 = [(8, 8, 0)] + [(0, 1 << k, 0) for k in range(4, BLOG)]   # 16 + (B - 16) bytes; BLOG - 3 = 11 matches at 16 KiB
     lits0 = b"ABCDEFGH"
-    lits1 = b"0123456789" + bytes((i * 7 + 3) & 0xFF for i in range(300)) + b"tail" * 4014 + b"xy"
+    lits1 = b"0123456789" + bytes((i * 7 + 3) & 0xFF for i in range(300)) + b"tail" * ((B - 328) // 4) + b"xy"
     seqs1 = [(10, 12, B - 5), (300, 4, 3)]
     assert 10 + 12 + 300 + 4 + (len(lits1) - 310) == B
     seqs2 = [(0, 100, B + 10)]
@@ -42,12 +42,12 @@ def test_handmade_container_decodes_to_plain_definition():
             blk, hops = iso.decode(b, with_hops=True)
             assert blk.tobytes() == want[b * B:(b + 1) * B]
         # last byte of block 0 was produced by the 11th match: 11 hops back to a literal
-        assert iso.decode(0, with_hops=True)[1] == 11
+        assert iso.decode(0, with_hops=True)[1] == BLOG - 3
     ll, ml, src, tags = oracle.decode_tokens(c, 0)
-    assert list(tags) == list(range(1, 12)) and int(ml[-1]) == 8192
+    assert list(tags) == list(range(1, BLOG - 2)) and int(ml[-1]) == B // 2
     assert list(oracle.decode_tokens(c, 1)[3]) == [1, 0] and list(oracle.decode_tokens(c, 2)[3]) == [0]
     rep = oracle.validate(c)
-    assert rep.n_matches_spanning == 1 and rep.max_level_seen == 11 and rep.min_match_seen == 4
+    assert rep.n_matches_spanning == 1 and rep.max_level_seen == BLOG - 3 and rep.min_match_seen == 4
     h, lit, ln, off, ex, tg = oracle.decode_streams(c, 1)
     assert h.n_seq == 2 and h.n_extras == 1 and int(ex[0]) == 300 and list(ln) == [10, 8, 255, 0]
     assert h.off_nbytes == 2 and list(off) == [(B - 5) & 255, (B - 5) >> 8, 3, 0]
@@ -227,8 +227,8 @@ def test_rejects_bad_frequency_sum_and_length_mismatch():
 def test_validator_flags_wrong_tags_and_broken_promises():
     total, blocks = handmade_case()
     recs = [build_record(b * B, s, l) for b, (s, l) in enumerate(blocks)]
-    assert oracle.validate(build_container(total, recs)).n_seq == 14
-    wrong = [build_record(0, blocks[0][0], blocks[0][1], tags=[1] * 11)] + recs[1:]
+    assert oracle.validate(build_container(total, recs)).n_seq == BLOG
+    wrong = [build_record(0, blocks[0][0], blocks[0][1], tags=[1] * (BLOG - 3))] + recs[1:]
     with pytest.raises(oracle.OracleError) as e:
         oracle.validate(build_container(total, wrong))
     assert e.value.code == -7
