@@ -62,7 +62,8 @@ typedef struct {
     uint64_t total_len;      /* decompressed bytes */
     uint64_t n_blocks;       /* ceil(total_len / 16384) */
     uint64_t container_bytes;
-    uint32_t block_size;     /* 16384 */
+    uint32_t block_size;     /* 16384 (a library built with -DACEAPEX_BLOCK_LOG2=12..15 for the block-size sweep: 4096 .. 32768;
+                                every "16384" below then reads as this value) */
     uint32_t offset_width;   /* 4 or 8 */
     uint32_t max_depth;      /* header promise D (0 = none) */
     uint32_t window;         /* header promise R (0 = none) */
@@ -81,7 +82,8 @@ int aceapex_version(void);
  *   out          HOST, receives the context.
  * Validates the header (ACEAPEX_E_FORMAT) and runs one device pass over all block-record
  * headers (one entropy entry point per block) that checks them and finds the
- * largest n_seq; synchronises the device. A corrupt record header yields ACEAPEX_E_CORRUPT. */
+ * largest n_seq; synchronises the device. A corrupt record header yields ACEAPEX_E_CORRUPT.  * ACEAPEX_E_CAPACITY: the container's densest block needs more shared memory in the match kernel than the device
+ * offers (only reachable with 32 KiB blocks holding more than about 6,000 sequences). */
 int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, aceapex_ctx **out);
 
 /* HOST out. */
@@ -160,8 +162,8 @@ uint64_t aceapex_launch_count(const aceapex_ctx *ctx);
  * caller memory without running the match layer (the paper's harness checks the entropy layer
  * round trip on its own).
  *   d_lit  DEVICE, count*16384 bytes: block i's LIT stream at i*16384
- *   d_len  DEVICE, count*8192 bytes:  block i's LEN stream at i*8192
- *   d_off  DEVICE, count*32768 bytes: block i's OFF stream at i*32768
+ *   d_len  DEVICE, count*8192 bytes:  block i's LEN stream at i*8192   (block size / 2)
+ *   d_off  DEVICE, count*32768 bytes: block i's OFF stream at i*32768  (2 x block size)
  * count <= n_slots. */
 int aceapex_decode_streams(aceapex_ctx *ctx, uint64_t first, size_t count, void *d_lit, void *d_len,
                            void *d_off, void *cuda_stream);

@@ -14,7 +14,10 @@ import numpy as np
 
 from . import build as _build
 
-B = 16384
+# Block size: 16 KiB unless the library variant loaded through ACEAPEX_LIB was built for another one (block-size sweep,
+# `bench.py --sweep`), in which case ACEAPEX_BLOCK_LOG2 names it; aceapex_open rejects a container of any other size.
+BLOG = int(os.environ.get("ACEAPEX_BLOCK_LOG2", "14"))
+B = 1 << BLOG
 PACKED, ABSOLUTE = 0, 1
 
 ERRORS = {0: "OK", -1: "E_ARG", -2: "E_FORMAT", -3: "E_CAPACITY", -4: "E_CORRUPT", -5: "E_RANGE",
@@ -180,8 +183,8 @@ class Decoder:
     def decode_streams(self, first: int, count: int, stream=None):
         torch = self._torch
         lit = torch.zeros(count * B, dtype=torch.uint8, device=self.device)
-        ln = torch.zeros(count * 8192, dtype=torch.uint8, device=self.device)
-        off = torch.zeros(count * 32768, dtype=torch.uint8, device=self.device)
+        ln = torch.zeros(count * (B // 2), dtype=torch.uint8, device=self.device)
+        off = torch.zeros(count * (2 * B), dtype=torch.uint8, device=self.device)
         with torch.cuda.device(self.device):
             _check(lib().aceapex_decode_streams(self._ctx, first, count, lit.data_ptr(), ln.data_ptr(), off.data_ptr(),
                                                 _stream_ptr(stream)), "aceapex_decode_streams")

@@ -301,11 +301,20 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
     if (rc != ACEAPEX_OK) { aceapex_close(c); return rc; }
 
     c->sl = make_slot_layout(res.max_n_seq, c->cv.W);
-    // The attribute belongs to the function, not to this context: set it to the format maximum (4096 sequences,
-    // 8-byte offsets) so that contexts of different containers cannot lower each other's limit.
-    if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)match_smem_bytes(kMaxSeq, 8)) != cudaSuccess) {
-        aceapex_close(c);
-        return ACEAPEX_E_CUDA;
+    // The attribute belongs to the function, not to this context: set it to the format maximum (block size / 4
+    // sequences, 8-byte offsets), or to what the device offers if that is less (32 KiB blocks), so that contexts of
+    // different containers cannot lower each other's limit. A container whose densest block needs more than the
+    // device has cannot be decoded by this build.
+    {
+        int optin = 0;
+        if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { aceapex_close(c); return ACEAPEX_E_CUDA; }
+        const size_t avail = (size_t)optin > 2048 ? (size_t)optin - 2048 : 0;   // the kernel's static shared memory
+        const size_t fmt_max = match_smem_bytes(kMaxSeq, 8);
+        if (match_smem(c) > avail) { aceapex_close(c); return ACEAPEX_E_CAPACITY; }
+        if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(fmt_max < avail ? fmt_max : avail)) != cudaSuccess) {
+            aceapex_close(c);
+            return ACEAPEX_E_CUDA;
+        }
     }
     c->info.total_len = total_len;
     c->info.n_blocks = n_blocks;

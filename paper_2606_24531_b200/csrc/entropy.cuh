@@ -394,8 +394,8 @@ __global__ void k_export_streams(Container cv, SlotLayout sl, const uint8_t *slo
     if (!r.ok) return;
     const uint8_t *slot = slots + (size_t)bi * sl.stride;
     for (uint32_t i = threadIdx.x; i < r.n_sym[LIT]; i += blockDim.x) d_lit[(size_t)bi * kB + i] = slot[sl.o_lit + i];
-    for (uint32_t i = threadIdx.x; i < r.n_sym[LEN]; i += blockDim.x) d_len[(size_t)bi * 8192 + i] = slot[sl.o_len + i];
-    for (uint32_t i = threadIdx.x; i < r.n_sym[OFF]; i += blockDim.x) d_off[(size_t)bi * 32768 + i] = slot[sl.o_off + i];
+    for (uint32_t i = threadIdx.x; i < r.n_sym[LEN]; i += blockDim.x) d_len[(size_t)bi * (kB / 2) + i] = slot[sl.o_len + i];
+    for (uint32_t i = threadIdx.x; i < r.n_sym[OFF]; i += blockDim.x) d_off[(size_t)bi * (2 * kB) + i] = slot[sl.o_off + i];
 }
 
 }  // namespace aceapex

@@ -6,9 +6,16 @@
 
 namespace aceapex {
 
-constexpr uint32_t kBlockLog2 = 14;            // FORMAT.md section 1: block_log2
-constexpr uint32_t kB = 1u << kBlockLog2;      // 16384 bytes per block
-constexpr uint32_t kMaxSeq = 4096;             // n_seq <= 4096 (FORMAT.md section 2)
+// FORMAT.md section 1: block_log2. 14 = 16384 bytes per block; -DACEAPEX_BLOCK_LOG2=12..15 builds the
+// library for another block size (block-size sweep; `bench.py --sweep`). 16 would not fit the
+// record header's 16-bit n_lit, nor the 16-bit positions the kernels pack in pairs.
+#ifndef ACEAPEX_BLOCK_LOG2
+#define ACEAPEX_BLOCK_LOG2 14
+#endif
+constexpr uint32_t kBlockLog2 = ACEAPEX_BLOCK_LOG2;
+static_assert(kBlockLog2 >= 12 && kBlockLog2 <= 15, "block size 4 .. 32 KiB");
+constexpr uint32_t kB = 1u << kBlockLog2;
+constexpr uint32_t kMaxSeq = kB / 4;           // n_seq <= block size / 4: a sequence is at least 4 bytes (FORMAT.md section 2)
 constexpr uint32_t kLanes = 32;                // rANS lanes per stream
 constexpr uint32_t kProbBits = 12;             // 12-bit quantised frequencies
 constexpr uint32_t kM = 1u << kProbBits;       // 4096

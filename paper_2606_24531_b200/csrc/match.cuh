@@ -86,17 +86,18 @@ __device__ inline unsigned long long wait_for_blocks(Control *ctl, const uint32_
 // by pass 0 with whatever the buffer held and then rewritten level by level from a list sorted by tag.
 
 // Dynamic shared memory of one match CTA (bytes), for a slot capacity of ms sequences and offset width W:
-//   cb    uint2 [512]       {run-start bits of 32 output offsets, number of run starts before them}
+//   cb    uint2 [kB / 32]   {run-start bits of 32 output offsets, number of run starts before them}
 //   stage u8 [warps][512]   16-byte store staging, one 512-byte tile per warp
 //   delta u64 [2 ms + 2]    per run (at most 2 n + 1)
 //   dm    u32 [ms]          per sequence: dst | match_len << 16 (before the main pass: true lit_len | match_len << 16
 //                           of a block with length escapes)
 //   mrun  u16 [ms]          per sequence: run number of its match
-//   tlist u16 [ms]          tagged matches, unsorted: k | tag << 12
+//   tlist u16 [ms]          tagged matches, unsorted: the sequence number k (its tag is read again from the staged nibbles)
 //   len   u16 [ms]          staged LEN stream; after the parse: tag list sorted by level
 //   off   u8 [W ms + 16]    staged OFF stream (the word-wise offset read may touch 11 bytes past the last offset)
 //   tags  u8 [pad16(ms/2)]  staged tag nibbles
-constexpr uint32_t kMatchFixedSmem = 4096 + kMatchWarps * 512;
+constexpr uint32_t kCbWords = kB / 32;                              // 512 at 16 KiB
+constexpr uint32_t kMatchFixedSmem = kCbWords * 8 + kMatchWarps * 512;
 
 __host__ __device__ inline uint32_t match_smem_bytes(uint32_t ms, uint32_t W)
 {
@@ -230,8 +231,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     __shared__ uint32_t s_cnt[16], s_cur[16];
 
     const uint32_t ms = sl.ms;
-    uint2 *cb = reinterpret_cast<uint2 *>(smem);                                    // [512]
-    uint8_t *stage = smem + 4096;                                                   // [kMatchWarps][512]
+    uint2 *cb = reinterpret_cast<uint2 *>(smem);                                    // [kCbWords]
+    uint8_t *stage = smem + kCbWords * 8;                                                   // [kMatchWarps][512]
     unsigned long long *delta = reinterpret_cast<unsigned long long *>(smem + kMatchFixedSmem);   // [2*ms+2]
     uint32_t *dm = reinterpret_cast<uint32_t *>(smem + kMatchFixedSmem + 16 * ms + 16);           // [ms]
     uint16_t *mrun = reinterpret_cast<uint16_t *>(dm + ms);                         // [ms]
@@ -244,7 +245,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t lt = (1u << lane) - 1u;
     const uint32_t out_aligned4 = out_align >= 4;
-    constexpr uint32_t kWordsPerThread = 512 / kMatchThreads;          // bitmap words per thread in the rank scan
+    constexpr uint32_t kWordsPerThread = kCbWords >= kMatchThreads ? kCbWords / kMatchThreads : 1;   // rank scan
+    static_assert(kCbWords % kWordsPerThread == 0, "bitmap words per thread");
   // Persistent CTAs: each takes block after block from the ticket counter until none is left.
   for (;;) {
     __syncthreads();                                                   // the previous block's shared state is dead
@@ -255,7 +257,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
         s_bad = 0;
     }
     if (tid < 16) s_cnt[tid] = 0;
-    for (uint32_t i = tid; i < 256; i += kMatchThreads) reinterpret_cast<uint4 *>(cb)[i] = make_uint4(0, 0, 0, 0);
+    for (uint32_t i = tid; i < kCbWords / 2; i += kMatchThreads) reinterpret_cast<uint4 *>(cb)[i] = make_uint4(0, 0, 0, 0);
     __syncthreads();
     if (s_ticket > count) break;                                       // tickets 1 .. count are blocks
     if (s_ticket == 0) {
@@ -455,7 +457,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                         if (lane == 0) tb = atomicAdd(&s_ntag, (uint32_t)__popc(tm));
                         tb = __shfl_sync(0xFFFFFFFFu, tb, 0);
                         if (tg) {
-                            tlist[tb + __popc(tm & lt)] = (uint16_t)(k | tg << 12);
+                            tlist[tb + __popc(tm & lt)] = (uint16_t)k;
                             atomicAdd(&s_cnt[tg], 1u);
                         }
                     }
@@ -479,11 +481,12 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             // cb[w].y = number of run starts in the words before w; tag list sorted by level
             {
                 uint32_t p[kWordsPerThread], tot = 0;
+                const bool mine = kWordsPerThread * tid < kCbWords;    // (a 4 KiB block has fewer words than threads)
 #pragma unroll
-                for (uint32_t i = 0; i < kWordsPerThread; i++) { p[i] = __popc(cb[kWordsPerThread * tid + i].x); tot += p[i]; }
+                for (uint32_t i = 0; i < kWordsPerThread; i++) { p[i] = mine ? __popc(cb[kWordsPerThread * tid + i].x) : 0u; tot += p[i]; }
                 uint32_t r0 = block_excl_scan(tot, ws1);
 #pragma unroll
-                for (uint32_t i = 0; i < kWordsPerThread; i++) { cb[kWordsPerThread * tid + i].y = r0; r0 += p[i]; }
+                for (uint32_t i = 0; i < kWordsPerThread; i++) { if (mine) cb[kWordsPerThread * tid + i].y = r0; r0 += p[i]; }
             }
             const uint32_t ntag = s_ntag;
             const bool one_level = s_cnt[1] == ntag;                   // every tagged match has tag 1: no sorting
@@ -496,8 +499,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                 }
                 __syncthreads();
                 for (uint32_t i = tid; i < ntag; i += kMatchThreads) {
-                    const uint32_t e = tlist[i];
-                    slist[atomicAdd(&s_cur[e >> 12], 1u)] = (uint16_t)e;
+                    const uint32_t k = tlist[i];
+                    slist[atomicAdd(&s_cur[(s_tags[k >> 1] >> ((k & 1) * 4)) & 15u], 1u)] = (uint16_t)k;
                 }
                 lst = slist;
             }
@@ -576,7 +579,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
                             const uint32_t i = ib + u * G;
                             ml[u] = 0; sp[u] = dp[u] = 0;
                             if (i < i1) {
-                                const uint32_t k = lst[i] & 0xFFFu;
+                                const uint32_t k = lst[i];
                                 const uint32_t dmv = dm[k], d = dmv & 0xFFFFu;
                                 ml[u] = dmv >> 16;
                                 sp[u] = delta[mrun[k]] + d; dp[u] = outB + d;
