@@ -123,6 +123,35 @@ __device__ inline uint32_t shl_clamp(uint32_t v, uint32_t s)   // PTX shl: shift
     return r;
 }
 
+// ---- bulk async copies (TMA, sm_90+: cp.async.bulk, SASS UBLKCP) completing on a shared-memory mbarrier --------
+// One thread posts the expected byte count and issues the copies; every thread then waits for the barrier's phase.
+__device__ inline uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ inline void mbar_init(unsigned long long *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ inline void mbar_expect_tx(unsigned long long *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ inline void bulk_copy_g2s(void *dst_smem, const void *src, uint32_t bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ inline void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "MBAR_WAIT:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra MBAR_DONE;\n"
+                 "bra MBAR_WAIT;\n"
+                 "MBAR_DONE:\n"
+                 "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
 // Exclusive prefix sum of one value per thread over the CTA.
 __device__ inline uint32_t block_excl_scan(uint32_t a, uint32_t *ws /* [kMatchWarps] smem */)
 {
@@ -229,6 +258,7 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     __shared__ uint32_t s_ticket, s_ntag, s_bad;
     __shared__ unsigned long long s_wm, s_last;
     __shared__ uint32_t s_cnt[16], s_cur[16];
+    __shared__ __align__(8) unsigned long long s_mbar;                 // completion of a block's staging copies
 
     const uint32_t ms = sl.ms;
     uint2 *cb = reinterpret_cast<uint2 *>(smem);                                    // [kCbWords]
@@ -247,6 +277,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
     const uint32_t out_aligned4 = out_align >= 4;
     constexpr uint32_t kWordsPerThread = kCbWords >= kMatchThreads ? kCbWords / kMatchThreads : 1;   // rank scan
     static_assert(kCbWords % kWordsPerThread == 0, "bitmap words per thread");
+    if (tid == 0) mbar_init(&s_mbar, 1);
+    uint32_t stage_phase = 0;                                          // parity of the staging barrier's current phase
   // Persistent CTAs: each takes block after block from the ticket counter until none is left.
   for (;;) {
     __syncthreads();                                                   // the previous block's shared state is dead
@@ -311,17 +343,24 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
             // one packed warp scan per round plus a carry.
             const uint32_t cw = ((n + kMatchThreads - 1) / kMatchThreads) * 32;
             const uint32_t wk0 = min(n, warp * cw), wk1 = min(n, wk0 + cw);
-            // Stage the decoded LEN / OFF streams and the tag nibbles into shared memory with one round of
-            // 16-byte async copies (sizes padded to 16 stay inside the slot areas / the record).
-            {
-                const uint32_t nl = (2 * n + 15) >> 4, no = (r.off_nbytes * n + 15) >> 4, nt = ((n + 1) / 2 + 15) >> 4;
-                const uint8_t *gl = slot + sl.o_len, *go = slot + sl.o_off, *gt = r.rec + r.tags_off;
-                for (uint32_t i = tid; i < nl; i += kMatchThreads) cp_async16(reinterpret_cast<uint8_t *>(s_len16) + 16 * i, gl + 16 * i);
-                for (uint32_t i = tid; i < no; i += kMatchThreads) cp_async16(s_off + 16 * i, go + 16 * i);
-                for (uint32_t i = tid; i < nt; i += kMatchThreads) cp_async16(s_tags + 16 * i, gt + 16 * i);
-                cp_async_commit();
+            // Stage the decoded LEN / OFF streams and the tag nibbles into shared memory: three bulk async copies
+            // (TMA: one instruction per stream, issued by one thread, completing on a shared-memory mbarrier; the
+            // sizes padded to 16 stay inside the slot areas / the record) instead of a cp.async loop over all threads.
+            if (n) {
+                const uint32_t nl = (2 * n + 15) & ~15u, no = (r.off_nbytes * n + 15) & ~15u, nt = ((n + 1) / 2 + 15) & ~15u;
+                if (tid == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the previous block's reads of these buffers are done (loop-top barrier)
+                    mbar_expect_tx(&s_mbar, nl + no + nt);
+                    bulk_copy_g2s(s_len16, slot + sl.o_len, nl, &s_mbar);
+                    bulk_copy_g2s(s_off, slot + sl.o_off, no, &s_mbar);
+                    bulk_copy_g2s(s_tags, r.rec + r.tags_off, nt, &s_mbar);
+                }
                 if (tid == kMatchThreads - 1) s_wm = ld_acquire_u64(&ctl->watermark);   // it only grows; overlapped with the copies
-                cp_async_wait_all();
+                if (warp == 0) mbar_wait(&s_mbar, stage_phase);       // one warp polls; the others sleep in the CTA barrier
+                stage_phase ^= 1u;
+                __syncthreads();                                       // (also publishes s_wm)
+            } else {
+                if (tid == kMatchThreads - 1) s_wm = ld_acquire_u64(&ctl->watermark);
                 __syncthreads();
             }
             const uint16_t *len16 = s_len16;
