@@ -99,7 +99,7 @@ uint32_t match_grid(aceapex_ctx *c, uint32_t count)
 {
     if (c->match_ctas_per_sm == 0) {
         int nb = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_match, (int)kMatchThreads, match_smem(c)) != cudaSuccess || nb < 1) nb = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_match<16>, (int)kMatchThreads, match_smem(c)) != cudaSuccess || nb < 1) nb = 1;
         c->match_ctas_per_sm = nb;
     }
     const uint64_t cap = (uint64_t)c->match_ctas_per_sm * (uint64_t)c->sm_count;
@@ -201,7 +201,12 @@ int decode_span(aceapex_ctx *c, uint64_t first, uint64_t count, uint8_t *d_out, 
         if (rc != ACEAPEX_OK) return rc;
         {
             LaunchScope ls(c, K_MATCH, st);
-            k_match<<<match_grid(c, cnt), kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, f, cnt, out_virtual, align,
+            const uint32_t grid = match_grid(c, cnt);
+            if (align >= 16) k_match<16><<<grid, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, f, cnt, out_virtual,
+                                                                    c->sc.ctl, c->sc.done, c->epoch, range_lo);
+            else if (align >= 4) k_match<4><<<grid, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, f, cnt, out_virtual,
+                                                                    c->sc.ctl, c->sc.done, c->epoch, range_lo);
+            else k_match<1><<<grid, kMatchThreads, match_smem(c), st>>>(c->cv, c->sl, c->sc.slots, f, cnt, out_virtual,
                                                                     c->sc.ctl, c->sc.done, c->epoch, range_lo);
         }
         if (cudaGetLastError() != cudaSuccess) return ACEAPEX_E_CUDA;
@@ -311,7 +316,9 @@ int aceapex_open(const void *d_container, size_t nbytes, const void *h_header, a
         const size_t avail = (size_t)optin > 2048 ? (size_t)optin - 2048 : 0;   // the kernel's static shared memory
         const size_t fmt_max = match_smem_bytes(kMaxSeq, 8);
         if (match_smem(c) > avail) { aceapex_close(c); return ACEAPEX_E_CAPACITY; }
-        if (cudaFuncSetAttribute(k_match, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(fmt_max < avail ? fmt_max : avail)) != cudaSuccess) {
+        if (cudaFuncSetAttribute(k_match<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(fmt_max < avail ? fmt_max : avail)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_match<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(fmt_max < avail ? fmt_max : avail)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_match<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(fmt_max < avail ? fmt_max : avail)) != cudaSuccess) {
             aceapex_close(c);
             return ACEAPEX_E_CUDA;
         }

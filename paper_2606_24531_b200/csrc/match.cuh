@@ -247,9 +247,12 @@ __device__ inline void stg_v4(unsigned long long a, uint4 v)
     asm volatile("st.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
+// kOutAlign: alignment of the output buffer (16, 4 or 1), a template parameter so that each instantiation carries one
+// store path (measured on mixed_1g: k_match 2.20 -> 2.07 ms against the run-time switch).
+template <uint32_t kOutAlign>
 __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayout sl, const uint8_t *slots,
                                                           uint64_t first, uint32_t count, uint8_t *out,
-                                                          uint32_t out_align /* 16, 4 or 1 */, Control *ctl, uint32_t *done,
+                                                          Control *ctl, uint32_t *done,
                                                           uint32_t epoch, uint64_t range_lo)
 {
     extern __shared__ __align__(16) uint8_t smem[];
@@ -274,7 +277,8 @@ __global__ void __launch_bounds__(kMatchThreads) k_match(Container cv, SlotLayou
 
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t lt = (1u << lane) - 1u;
-    const uint32_t out_aligned4 = out_align >= 4;
+    constexpr uint32_t out_align = kOutAlign;
+    constexpr uint32_t out_aligned4 = out_align >= 4;
     constexpr uint32_t kWordsPerThread = kCbWords >= kMatchThreads ? kCbWords / kMatchThreads : 1;   // rank scan
     static_assert(kCbWords % kWordsPerThread == 0, "bitmap words per thread");
     if (tid == 0) mbar_init(&s_mbar, 1);
