@@ -183,6 +183,32 @@ const char *aceapex_strerror(int code);
 
 void aceapex_close(aceapex_ctx *ctx);
 
+/* aceapex_decode_all_static: aceapex_decode_all for callers that cannot allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc). No context, no caller scratch: the whole decode - both
+ * layers of every block, PAPER.md:76 - is enqueued on `cuda_stream` by this one call, which allocates nothing (no
+ * cudaMalloc / cudaFree, no host allocation), never synchronises and reads nothing back. The kernels' scratch (control
+ * words, done flags, the slots with the decoded token streams) lives in ONE file-scope array in device memory of
+ * ACEAPEX_STATIC_SCRATCH_BYTES (8 MiB), which every GPU that loads the library holds until the process exits.
+ *   d_container  DEVICE, 16-byte aligned, `nbytes` long; FORMAT.md container.
+ *   h_header     HOST, the container's first 64 bytes (required: the call does not read the device).
+ *   max_n_seq    upper bound on the sequences per block of this container (aceapex_info.max_n_seq of an earlier
+ *                aceapex_open, or what the encoder promised); 0 = the format maximum (block size / 4), which costs
+ *                speed and slots. A block with more sequences is left unwritten and reported in d_status.
+ *   d_out        DEVICE, capacity `out_capacity` >= total_len; receives out[0, total_len).
+ *   d_status     DEVICE, optional, 32 bytes, 8-byte aligned: after the decode the stream copies there
+ *                { u64 first_bad_block (~0 = none), u64 blocks_complete, u64 reserved, u32 status (0 = ok, else the
+ *                sticky bits of a corrupt container), u32 reserved }.
+ * Limits (else ACEAPEX_E_CAPACITY, nothing enqueued): at most ACEAPEX_STATIC_MAX_BLOCKS (4,096) blocks = 64 MiB of
+ * output, and the bookkeeping plus at least one slot must fit the array; the blocks are decoded in sub-batches of
+ * as many slots as fit (about 230 at max_n_seq 1,000). Other errors: ACEAPEX_E_ARG, ACEAPEX_E_FORMAT
+ * (header), ACEAPEX_E_CUDA. The array is shared by ALL calls of a process on that GPU and keeps the last call's
+ * contents: every call clears what must start at zero on its stream first, so calls in stream order are
+ * independent - but two calls that overlap on the GPU (different streams, or graphs launched concurrently) race
+ * on it and corrupt each other. Matches the output of aceapex_decode_all bit for bit. */
+enum { ACEAPEX_STATIC_SCRATCH_BYTES = 8 << 20, ACEAPEX_STATIC_MAX_BLOCKS = 4096 };
+int aceapex_decode_all_static(const void *d_container, size_t nbytes, const void *h_header, uint32_t max_n_seq,
+                              void *d_out, size_t out_capacity, void *d_status, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

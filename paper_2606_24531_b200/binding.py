@@ -28,7 +28,7 @@ E_ARG, E_FORMAT, E_CAPACITY, E_CORRUPT, E_RANGE, E_NOMEM, E_CUDA, E_STATE = -1, 
 SYMBOLS = ["aceapex_version", "aceapex_open", "aceapex_info_get", "aceapex_scratch_bytes", "aceapex_set_scratch",
            "aceapex_decode_all", "aceapex_decode_range", "aceapex_decode_blocks", "aceapex_seek", "aceapex_device_status",
            "aceapex_launch_count", "aceapex_decode_streams", "aceapex_profile_enable", "aceapex_profile_read",
-           "aceapex_kernel_name", "aceapex_strerror", "aceapex_close"]
+           "aceapex_kernel_name", "aceapex_strerror", "aceapex_close", "aceapex_decode_all_static"]
 N_KERNELS = 16
 
 
@@ -80,6 +80,7 @@ def lib():
             L.aceapex_kernel_name.argtypes = [C.c_int]; L.aceapex_kernel_name.restype = C.c_char_p
             L.aceapex_strerror.argtypes = [C.c_int]; L.aceapex_strerror.restype = C.c_char_p
             L.aceapex_close.argtypes = [vp]; L.aceapex_close.restype = None
+            L.aceapex_decode_all_static.argtypes = [vp, sz, vp, u32, vp, sz, vp, vp]
             _lib = L
     return _lib
 
@@ -239,3 +240,22 @@ class Decoder:
             self.close()
         except Exception:
             pass
+
+
+STATIC_SCRATCH_BYTES = 8 << 20
+STATIC_MAX_BLOCKS = 4096
+
+
+def decode_all_static(container, out, header, max_n_seq: int = 0, status=None, stream=None) -> None:
+    """aceapex_decode_all_static: the whole decode enqueued by one call that allocates nothing (the kernels' scratch
+    is a static device array of the library; at most STATIC_MAX_BLOCKS blocks; calls that overlap on the GPU race).
+    `container` / `out` / `status` (32 bytes, optional) are CUDA uint8 tensors, `header` the container's first 64
+    bytes on the host (bytes or a numpy array)."""
+    import torch
+    hdr = np.ascontiguousarray(np.frombuffer(bytes(header[:64]), dtype=np.uint8))
+    if hdr.size != 64:
+        raise ValueError("header: the container's first 64 bytes")
+    with torch.cuda.device(container.device):
+        _check(lib().aceapex_decode_all_static(container.data_ptr(), container.numel(), hdr.ctypes.data, int(max_n_seq),
+                                               out.data_ptr(), out.numel(), status.data_ptr() if status is not None else None,
+                                               _stream_ptr(stream)), "aceapex_decode_all_static")

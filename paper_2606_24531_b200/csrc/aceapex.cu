@@ -5,6 +5,7 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -509,5 +510,126 @@ int aceapex_profile_read(aceapex_ctx *c, uint64_t *launches, double *ms)
 }
 
 const char *aceapex_kernel_name(int id) { return id >= 0 && id < K_COUNT ? kKernelNames[id] : nullptr; }
+
+// ---- aceapex_decode_all_static: decode_all without any allocation ------------------------------------------------
+//
+// The scratch of the two decode_all kernels in a file-scope device array instead of caller memory. In host code the
+// array's NAME is a host-side stand-in, not a device address (a kernel handed it would fault or use the wrong
+// memory): its address on the current device comes from cudaGetSymbolAddress, once per device.
+static __device__ __align__(256) unsigned char g_static_scratch[ACEAPEX_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMaxStaticDevices = 64;
+struct StaticDevice { bool ready; uint8_t *scratch; int sm_count; size_t smem_avail; };
+StaticDevice g_static_dev[kMaxStaticDevices];
+std::mutex g_static_mutex;
+
+// Set-up, once per device, with that device current: the array's device address, the kernels' shared-memory
+// attributes, the SM count. No allocation.
+int static_device(int dev, StaticDevice *out)
+{
+    if (dev < 0 || dev >= kMaxStaticDevices) return ACEAPEX_E_ARG;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice &d = g_static_dev[dev];
+    if (!d.ready) {
+        void *ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) return ACEAPEX_E_CUDA;
+        int optin = 0;
+        if (cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+            return ACEAPEX_E_CUDA;
+        d.smem_avail = (size_t)optin > 2048 ? (size_t)optin - 2048 : 0;
+        const size_t fmt_max = match_smem_bytes(kMaxSeq, 8);
+        const int msm = (int)(fmt_max < d.smem_avail ? fmt_max : d.smem_avail);
+        if (cudaFuncSetAttribute(k_entropy, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)entropy_smem()) != cudaSuccess ||
+            cudaFuncSetAttribute(k_match<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, msm) != cudaSuccess ||
+            cudaFuncSetAttribute(k_match<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, msm) != cudaSuccess ||
+            cudaFuncSetAttribute(k_match<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, msm) != cudaSuccess)
+            return ACEAPEX_E_CUDA;
+        d.scratch = static_cast<uint8_t *>(ptr);
+        d.ready = true;
+    }
+    *out = d;
+    return ACEAPEX_OK;
+}
+
+}  // namespace
+
+int aceapex_decode_all_static(const void *d_container, size_t nbytes, const void *h_header, uint32_t max_n_seq,
+                              void *d_out, size_t out_capacity, void *d_status, void *cuda_stream)
+{
+    if (!d_container || !h_header || ((uintptr_t)d_container & 15) || ((uintptr_t)d_status & 7)) return ACEAPEX_E_ARG;
+    if (nbytes < kHeaderBytes) return ACEAPEX_E_FORMAT;
+    const uint8_t *h = static_cast<const uint8_t *>(h_header);
+    // FORMAT.md section 1 (the same checks as aceapex_open, from the caller's host copy of the header)
+    if (memcmp(h, "ACEAPEX1", 8) != 0 || rd32(h + 8) != 1) return ACEAPEX_E_FORMAT;
+    if (h[12] != kBlockLog2 || (h[13] != 4 && h[13] != 8) || h[14] != kLanes || h[15] != kProbBits) return ACEAPEX_E_FORMAT;
+    const uint64_t total_len = rd64(h + 16), n_blocks = rd64(h + 24);
+    const uint64_t index_off = rd64(h + 48), payload_off = rd64(h + 56);
+    if (n_blocks != (total_len + kB - 1) / kB || n_blocks > (1ull << 32) - 2) return ACEAPEX_E_FORMAT;
+    if (index_off != kHeaderBytes || rd32(h + 40) > 15) return ACEAPEX_E_FORMAT;
+    const uint64_t index_bytes = (n_blocks + 1) * 8 + n_blocks * 3 * kLanes * 4;
+    if (payload_off != ((kHeaderBytes + index_bytes + 15) & ~15ull) || payload_off > nbytes) return ACEAPEX_E_FORMAT;
+    if (!d_out && total_len) return ACEAPEX_E_ARG;
+    if (out_capacity < total_len) return ACEAPEX_E_CAPACITY;
+    if (n_blocks > ACEAPEX_STATIC_MAX_BLOCKS) return ACEAPEX_E_CAPACITY;
+    if (max_n_seq == 0 || max_n_seq > kMaxSeq) max_n_seq = kMaxSeq;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return ACEAPEX_E_CUDA;
+    StaticDevice sd;
+    int rc = static_device(dev, &sd);
+    if (rc != ACEAPEX_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+    // a context on the stack (nothing in it allocates), its scratch carved out of the static array
+    aceapex_ctx c;
+    const uint8_t *base = static_cast<const uint8_t *>(d_container);
+    c.cv.base = base;
+    c.cv.rec_off = reinterpret_cast<const uint64_t *>(base + kHeaderBytes);
+    c.cv.states = reinterpret_cast<const uint32_t *>(base + kHeaderBytes + (n_blocks + 1) * 8);
+    c.cv.payload = base + payload_off;
+    c.cv.total_len = total_len;
+    c.cv.n_blocks = n_blocks;
+    c.cv.payload_bytes = nbytes - payload_off;         // upper bound: every record must end inside the caller's buffer
+    c.cv.W = h[13]; c.cv.D = rd32(h + 32); c.cv.R = rd32(h + 36); c.cv.max_level = rd32(h + 40);
+    c.device = dev;
+    c.sm_count = sd.sm_count;
+    c.sl = make_slot_layout(max_n_seq, c.cv.W);
+    if (match_smem(&c) > sd.smem_avail) return ACEAPEX_E_CAPACITY;
+    if (n_blocks == 0) {
+        if (d_status && cudaMemsetAsync(d_status, 0, 32, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        if (d_status && cudaMemsetAsync(d_status, 0xFF, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+        return ACEAPEX_OK;
+    }
+    // as many slots as fit the array beside the bookkeeping (at most one per block)
+    const ScratchOffsets o1 = scratch_offsets(n_blocks, c.sl, 1, 0);
+    if (o1.total > ACEAPEX_STATIC_SCRATCH_BYTES) return ACEAPEX_E_CAPACITY;
+    size_t n_slots = 1 + (ACEAPEX_STATIC_SCRATCH_BYTES - o1.total) / ((size_t)c.sl.stride + 8);
+    if (n_slots > n_blocks) n_slots = (size_t)n_blocks;
+    while (n_slots > 1 && scratch_offsets(n_blocks, c.sl, n_slots, 0).total > ACEAPEX_STATIC_SCRATCH_BYTES) n_slots--;
+    const ScratchOffsets o = scratch_offsets(n_blocks, c.sl, n_slots, 0);
+    uint8_t *p = sd.scratch;
+    c.sc.ctl = reinterpret_cast<Control *>(p + o.ctl);
+    c.sc.done = reinterpret_cast<uint32_t *>(p + o.done);
+    c.sc.mark = reinterpret_cast<uint32_t *>(p + o.mark);
+    c.sc.slot_of = reinterpret_cast<unsigned long long *>(p + o.slot_of);
+    c.sc.list = reinterpret_cast<uint64_t *>(p + o.list);
+    c.sc.ids = reinterpret_cast<uint64_t *>(p + o.ids);
+    c.sc.slots = p + o.slots;
+    c.sc.pend = reinterpret_cast<uint64_t *>(p + o.pend);
+    c.sc.n_slots = n_slots;
+    c.sc.n_targets = 0;
+    c.have_scratch = true;
+    // The array keeps the previous call's contents: the control words (status, counters) and the done flags must
+    // start at zero, first_bad at ~0. (The slots are fully rewritten by the entropy kernel before they are read.)
+    if (cudaMemsetAsync(p, 0, o.mark, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    if (cudaMemsetAsync(&c.sc.ctl->first_bad, 0xFF, 8, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    rc = decode_span(&c, 0, n_blocks, static_cast<uint8_t *>(d_out), st);
+    if (rc != ACEAPEX_OK) return rc;
+    if (d_status && cudaMemcpyAsync(d_status, c.sc.ctl, 32, cudaMemcpyDeviceToDevice, st) != cudaSuccess) return ACEAPEX_E_CUDA;
+    return ACEAPEX_OK;
+}
 
 }  // extern "C"
