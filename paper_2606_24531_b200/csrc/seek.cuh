@@ -264,7 +264,9 @@ __global__ void __launch_bounds__(32 * kEntropyWarps, 2) k_seek_fused(Container 
     }
     const uint32_t n_ctas = gridDim.x;
     const uint64_t n_thr = (uint64_t)n_ctas * blockDim.x, gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint32_t n_warps = n_ctas * kEntropyWarps, gwarp = blockIdx.x * kEntropyWarps + warp;
+    // Warp numbering CTA-minor: consecutive work items go to different SMs, so a seek that touches a few hundred
+    // blocks runs one or two stream decodes per SM (each near its single-warp latency) instead of sixteen on a few SMs.
+    const uint32_t n_warps = n_ctas * kEntropyWarps, gwarp = warp * n_ctas + blockIdx.x;
     const uint64_t n_bytes = (uint64_t)a.nt * kB;
 
     // init: every target byte chases its own position; the first round's claims are the targets themselves
