@@ -61,7 +61,8 @@ class EncStats(C.Structure):
     _fields_ = [("n_seq", C.c_uint64), ("n_lit", C.c_uint64), ("match_bytes", C.c_uint64),
                 ("intra_match_bytes", C.c_uint64), ("n_extras", C.c_uint64),
                 ("n_sym", C.c_uint64 * 3), ("n_words", C.c_uint64 * 3), ("table_bytes", C.c_uint64),
-                ("max_depth_seen", C.c_uint32), ("max_level_seen", C.c_uint32), ("n_raw", C.c_uint64 * 3)]
+                ("max_depth_seen", C.c_uint32), ("max_level_seen", C.c_uint32), ("n_raw", C.c_uint64 * 3),
+                ("n_const", C.c_uint64 * 3)]
 
 
 class Info(C.Structure):

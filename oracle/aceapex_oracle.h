@@ -88,6 +88,7 @@ typedef struct {
     uint64_t n_sym[3], n_words[3], table_bytes;
     uint32_t max_depth_seen, max_level_seen;
     uint64_t n_raw[3];     /* streams stored RAW, per stream id */
+    uint64_t n_const[3];   /* streams stored CONST, per stream id */
 } ora_enc_stats;
 
 /* the block_log2 this library was compiled for (14 unless built with -DORA_BLOG) */

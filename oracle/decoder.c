@@ -79,7 +79,9 @@ int ora_record_open(const ora_container *k, uint64_t block, ora_record *r)
     }
     if (r->n_seq > ORA_MAX_SEQ || r->n_lit > r->block_len) return ORA_E_CORRUPT;
     if (r->off_nbytes < 1 || r->off_nbytes > k->info.offset_width) return ORA_E_CORRUPT;
-    if (r->modes & ~0x15u) return ORA_E_CORRUPT; /* per stream 2 bits: 0 = rANS, 1 = RAW; 2, 3 reserved */
+    /* per stream 2 bits: 0 = rANS, 1 = RAW, 2 = CONST; 3 and bits 6-7 reserved */
+    if (r->modes & 0xC0u) return ORA_E_CORRUPT;
+    for (int s = 0; s < 3; s++) if (((r->modes >> (2 * s)) & 3u) == 3u) return ORA_E_CORRUPT;
     if (r->n_extras > 2 * r->n_seq) return ORA_E_CORRUPT;
     r->n_sym[ORA_LIT] = r->n_lit;
     r->n_sym[ORA_LEN] = 2 * r->n_seq;
@@ -89,8 +91,11 @@ int ora_record_open(const ora_container *k, uint64_t block, ora_record *r)
         pos = pad16(pos);
         r->table[s] = rec + pos;
         pos += r->tbl_bytes[s];
-        if ((r->modes >> (2 * s)) & 1u) {       /* RAW: no table, the symbols sit in the words section */
+        const uint32_t mode = (r->modes >> (2 * s)) & 3u;
+        if (mode == 1u) {                       /* RAW: no table, the symbols sit in the words section */
             if (r->n_sym[s] == 0 || r->tbl_bytes[s] != 0 || r->n_words[s] != (r->n_sym[s] + 1) / 2) return ORA_E_CORRUPT;
+        } else if (mode == 2u) {                /* CONST: no table, one word whose low byte is the symbol */
+            if (r->n_sym[s] == 0 || r->tbl_bytes[s] != 0 || r->n_words[s] != 1) return ORA_E_CORRUPT;
         } else {
             if ((r->n_sym[s] == 0) != (r->tbl_bytes[s] == 0)) return ORA_E_CORRUPT;
             if (r->n_words[s] > r->n_sym[s]) return ORA_E_CORRUPT;
@@ -131,7 +136,13 @@ int ora_table_read(const uint8_t *tbl, uint32_t tbl_bytes, uint16_t freq[256])
 static int stream_decode(const ora_record *r, int s, uint8_t *out)
 {
     uint16_t freq[256];
-    if ((r->modes >> (2 * s)) & 1u) {           /* RAW (FORMAT.md section 2): copy; states unused, must be 2^16 */
+    if (((r->modes >> (2 * s)) & 3u) == 2u) {   /* CONST (FORMAT.md section 2): n_sym copies of one symbol */
+        for (int l = 0; l < 32; l++) if (r->states[s][l] != 65536u) return ORA_E_CORRUPT;
+        if (r->words[s][1] != 0) return ORA_E_CORRUPT;                                    /* high byte of the word */
+        memset(out, r->words[s][0], r->n_sym[s]);
+        return ORA_OK;
+    }
+    if (((r->modes >> (2 * s)) & 3u) == 1u) {   /* RAW (FORMAT.md section 2): copy; states unused, must be 2^16 */
         for (int l = 0; l < 32; l++) if (r->states[s][l] != 65536u) return ORA_E_CORRUPT;
         memcpy(out, r->words[s], r->n_sym[s]);
         if ((r->n_sym[s] & 1u) && r->words[s][r->n_sym[s]] != 0) return ORA_E_CORRUPT;   /* pad byte of the last word */

@@ -327,9 +327,17 @@ static int serialise_block(const enc_ctx *e, uint64_t b, enc_scratch *s, uint32_
         int rc = ora_rans_encode(sym[k], n_sym[k], freq, 32, out->states[k], s->words[k], &n_words[k]);
         if (rc != ORA_OK) return rc;
         if (n_sym[k]) tbl_bytes[k] = table_write(tables[k], freq);
-        /* selective entropy ("apply ANS selectively"; FORMAT.md section 2 modes): keep the
-         * stream verbatim when rANS does not pay for itself */
-        if (n_sym[k] && e->p.raw_slack_pct != 0xFFFFFFFFu &&
+        /* selective entropy ("apply ANS selectively"; FORMAT.md section 2 modes): a stream of one
+         * repeated symbol is stored as that symbol (CONST); otherwise keep the stream verbatim (RAW) when rANS does
+         * not pay for itself */
+        if (n_sym[k] && e->p.raw_slack_pct != 0xFFFFFFFFu && count[sym[k][0]] == n_sym[k]) {
+            modes |= 2u << (2 * k);
+            tbl_bytes[k] = 0;
+            n_words[k] = 1;
+            s->words[k][0] = sym[k][0];
+            for (int l = 0; l < 32; l++) out->states[k][l] = 65536u;
+            out->st.n_const[k]++;
+        } else if (n_sym[k] && e->p.raw_slack_pct != 0xFFFFFFFFu &&
             (uint64_t)n_sym[k] * 100 <= ((uint64_t)tbl_bytes[k] + 2 * (uint64_t)n_words[k]) * (100 + (uint64_t)e->p.raw_slack_pct)) {
             modes |= 1u << (2 * k);
             tbl_bytes[k] = 0;
@@ -474,7 +482,7 @@ int ora_encode(const uint8_t *in, size_t n, const ora_enc_params *pp, uint8_t *o
             const ora_enc_stats *t = &blocks[b].st;
             S.n_seq += t->n_seq; S.n_lit += t->n_lit; S.match_bytes += t->match_bytes;
             S.intra_match_bytes += t->intra_match_bytes; S.n_extras += t->n_extras; S.table_bytes += t->table_bytes;
-            for (int k = 0; k < 3; k++) { S.n_sym[k] += t->n_sym[k]; S.n_words[k] += t->n_words[k]; S.n_raw[k] += t->n_raw[k]; }
+            for (int k = 0; k < 3; k++) { S.n_sym[k] += t->n_sym[k]; S.n_words[k] += t->n_words[k]; S.n_raw[k] += t->n_raw[k]; S.n_const[k] += t->n_const[k]; }
             if (t->max_depth_seen > S.max_depth_seen) S.max_depth_seen = t->max_depth_seen;
             if (t->max_level_seen > S.max_level_seen) S.max_level_seen = t->max_level_seen;
         }

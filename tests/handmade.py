@@ -69,7 +69,13 @@ def _raw_stream(sym: bytes):
     return b"", body, len(body) // 2, [65536] * 32
 
 
-def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off_nbytes=None, freqs=None, raw=()):
+def _const_stream(sym: bytes):
+    """FORMAT.md section 2, mode 2 (CONST): no table, one word whose low byte is the repeated symbol."""
+    assert len(sym) >= 1 and len(set(sym)) == 1
+    return b"", bytes([sym[0], 0]), 1, [65536] * 32
+
+
+def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off_nbytes=None, freqs=None, raw=(), const=()):
     """seqs: list of (lit_len, match_len, src). `literals`: all literal bytes of the block.
     raw: names of the streams ("lit", "len", "off") to store RAW instead of rANS-coded."""
     if tags is None:
@@ -91,8 +97,9 @@ def build_record(block_start, seqs, literals: bytes, off_width=4, tags=None, off
         off_sym += int(src).to_bytes(8, "little")[:off_nbytes]
     freqs = freqs or {}
     syms = {"lit": bytes(literals), "len": bytes(len_sym), "off": bytes(off_sym)}
-    streams = [_raw_stream(syms[k]) if k in raw else _stream(syms[k], freqs.get(k)) for k in ("lit", "len", "off")]
-    modes = sum(1 << (2 * i) for i, k in enumerate(("lit", "len", "off")) if k in raw)
+    streams = [_raw_stream(syms[k]) if k in raw else (_const_stream(syms[k]) if k in const else _stream(syms[k], freqs.get(k)))
+               for k in ("lit", "len", "off")]
+    modes = sum((1 if k in raw else 2) << (2 * i) for i, k in enumerate(("lit", "len", "off")) if k in raw or k in const)
     hdr = struct.pack("<HHHBB", len(seqs), len(literals), len(extras), off_nbytes, modes)
     hdr += struct.pack("<III", *(s[2] for s in streams))
     hdr += struct.pack("<HHH", *(len(s[0]) for s in streams))

@@ -298,7 +298,7 @@ def test_rejects_inconsistent_raw_streams():
         with pytest.raises(oracle.OracleError):
             oracle.decode_all(c)
 
-    bad = good.copy(); bad[i.payload_off + 7] = 0x08                      # reserved mode 2 for LEN
+    bad = good.copy(); bad[i.payload_off + 7] = 0x0C                      # reserved mode 3 for LEN
     rejected(bad)
     bad = good.copy(); bad[i.payload_off + 7] |= 0x40                     # reserved bits 6-7
     rejected(bad)
@@ -372,3 +372,74 @@ def test_max_seq_caps_sequences_per_block():
     n0 = [oracle.decode_streams(c0, b)[0].n_seq for b in range(64)]
     n1 = [oracle.decode_streams(c1, b)[0].n_seq for b in range(64)]
     assert max(n0) > 300 and max(n1) == 300 and st1.n_seq < st0.n_seq and c1.size > c0.size
+
+
+# ---- selective entropy: CONST streams (FORMAT.md section 2 mode 2; SURVEY.md section 8f rank 1 "RAW / CONST / rANS")
+
+def const_case():
+    """2 blocks whose streams are constant by construction: block 0 is B equal literals (LIT constant, no sequences);
+    block 1 repeats the sequence (5 literals 'y', a 9-byte copy of out[7..16)) so that LIT, LEN (5, 5) and OFF (7, one
+    byte) are all constant streams."""
+    k = B // 14
+    blocks = [([], b"q" * B), ([(5, 9, 7)] * k, b"y" * (5 * k + (B - 14 * k)))]
+    return 2 * B, blocks
+
+
+def test_const_streams_decode_to_plain_definition():
+    total, blocks = const_case()
+    want = expand(total, blocks)
+    assert want[:B] == b"q" * B and want[B:B + 14] == b"yyyyy" + b"q" * 9
+    for const in [("lit",), ("len",), ("off",), ("lit", "len", "off")]:
+        recs = []
+        for b, (seqs, lits) in enumerate(blocks):
+            use = tuple(k for k in const if k == "lit" or seqs)           # block 0 has no LEN / OFF symbols at all
+            recs.append(build_record(b * B, seqs, lits, const=use))
+        c = build_container(total, recs)
+        assert oracle.decode_all(c).tobytes() == want, const
+        with oracle.Isolated(c) as iso:
+            for b in range(2):
+                assert iso.decode(b).tobytes() == want[b * B:(b + 1) * B]
+        oracle.validate(c)
+        h, lit, ln, off, ex, tg = oracle.decode_streams(c, 1)
+        assert set(ln) == {5} and set(off) == {7} and h.off_nbytes == 1 and set(lit) == {ord("y")}
+    # a constant stream costs one word instead of a 34-byte table
+    plain = build_container(total, [build_record(b * B, s, l) for b, (s, l) in enumerate(blocks)])
+    assert c.size < plain.size
+
+
+def test_encoder_stores_one_symbol_streams_as_const():
+    data = ADVERSARIAL["all_equal"]                                        # 3 blocks + 77 equal bytes
+    c, st = oracle.encode(data, return_stats=True)
+    assert np.array_equal(oracle.decode_all(c), np.frombuffer(data, np.uint8))
+    assert st.n_const[oracle.LIT] == 1 and sum(st.n_const) == 1            # block 0's four equal literals
+    c0, st0 = oracle.encode(data, return_stats=True, raw_slack_pct=0xFFFFFFFF)   # selective entropy off: rANS everywhere
+    assert sum(st0.n_const) == 0 and sum(st0.n_raw) == 0 and c.size < c0.size
+    assert np.array_equal(oracle.decode_all(c0), oracle.decode_all(c))
+    with oracle.Isolated(c) as iso:
+        for b in range(4):
+            assert iso.decode(b).tobytes() == data[b * B:(b + 1) * B]
+
+
+def test_rejects_inconsistent_const_streams():
+    total, blocks = const_case()
+    recs = [build_record(b * B, s, l, const=("lit",)) for b, (s, l) in enumerate(blocks)]
+    good = build_container(total, recs)
+    assert oracle.decode_all(good).tobytes() == expand(total, blocks)
+    i = oracle.info(good)
+
+    def rejected(c):
+        with pytest.raises(oracle.OracleError):
+            oracle.decode_all(c)
+
+    bad = good.copy(); bad[i.payload_off + 8] = 2                         # n_words[LIT] != 1
+    rejected(bad)
+    bad = good.copy(); bad[i.payload_off + 7] = 0x03                      # reserved mode 3 for LIT
+    rejected(bad)
+    bad = good.copy(); bad[i.payload_off + 20] = 34                       # a table section beside a CONST stream
+    rejected(bad)
+    bad = good.copy(); bad[64 + (i.n_blocks + 1) * 8 + 5 * 4] ^= 1        # block 0, LIT, lane 5: a state that is not 2^16
+    rejected(bad)
+    # block 0's record: header 32 bytes, no tables, no extras, no tags -> the LIT word sits at offset 32
+    assert good[i.payload_off + 32] == ord("q")
+    bad = good.copy(); bad[i.payload_off + 33] = 1                        # high byte of the word must be zero
+    rejected(bad)
