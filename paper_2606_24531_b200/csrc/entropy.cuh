@@ -282,6 +282,19 @@ __device__ inline bool copy_raw_stream(uint32_t x, uint32_t n, const uint8_t *wo
     return __all_sync(0xFFFFFFFFu, ok);
 }
 
+// A CONST stream (FORMAT.md section 2, mode 2): n copies of the symbol in the low byte of the stream's one word.
+// The stream areas of a slot are 16-byte aligned and padded, so the warp stores whole uint4s. The unused rANS states
+// must be 2^16 and the word's high byte 0.
+__device__ inline bool fill_const_stream(uint32_t x, uint32_t n, const uint8_t *words_sec, uint8_t *out, uint32_t lane)
+{
+    const uint32_t w = *reinterpret_cast<const uint16_t *>(words_sec);
+    const bool ok = x == kRansL && (w >> 8) == 0;
+    const uint32_t v = (w & 0xFFu) * 0x01010101u;
+    uint4 *dst = reinterpret_cast<uint4 *>(out);
+    for (uint32_t i = lane; i < (n + 15) >> 4; i += 32) dst[i] = make_uint4(v, v, v, v);
+    return __all_sync(0xFFFFFFFFu, ok);
+}
+
 // One (block, stream) unit, by one warp: stream s of block blk into slot bi. Output: the slot's stream
 // area and bad flag; with write_hdr also the record header fields in the slot header.
 __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, uint8_t *slots, uint64_t blk, uint32_t bi,
@@ -315,7 +328,8 @@ __device__ inline void decode_unit(const Container &cv, const SlotLayout &sl, ui
         const uint32_t wo = s == LIT ? r.words_off[LIT] : (s == LEN ? r.words_off[LEN] : r.words_off[OFF]);
         const uint32_t x0 = cv.states[(blk * 3 + (uint64_t)s) * kLanes + lane];
         const uint32_t is_raw = s == LIT ? r.raw[LIT] : (s == LEN ? r.raw[LEN] : r.raw[OFF]);
-        if (is_raw) ok = copy_raw_stream(x0, n, r.rec + wo, out, lane);
+        if (is_raw == 1u) ok = copy_raw_stream(x0, n, r.rec + wo, out, lane);
+        else if (is_raw == 2u) ok = fill_const_stream(x0, n, r.rec + wo, out, lane);
         else ok = decode_stream(x0, n, nw, r.rec + to, tb, r.rec + wo, out, ws, lane);
         if (!ok && leader()) raise(ctl, kStEntropy, blk);
     } else if (leader()) {

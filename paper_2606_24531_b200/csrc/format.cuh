@@ -44,7 +44,7 @@ struct Record {
     const uint8_t *rec;
     uint32_t block_len, n_seq, n_lit, n_extras, off_nbytes;
     uint32_t n_sym[3], n_words[3], tbl_bytes[3];
-    uint32_t raw[3];           // stream stored RAW (FORMAT.md section 2 modes; PAPER.md:94 selective entropy)
+    uint32_t raw[3];           // stream mode (FORMAT.md section 2; PAPER.md:94 selective entropy): 0 rANS, 1 RAW, 2 CONST
     uint32_t tbl_off[3], extras_off, tags_off, words_off[3];
     bool ok;
 };
@@ -89,8 +89,9 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
     r.tbl_bytes[OFF] = h1.z & 0xFFFFu;
     if (r.n_seq > kMaxSeq || r.n_lit > r.block_len) return r;
     if (r.off_nbytes < 1 || r.off_nbytes > cv.W) return r;
-    if (modes & ~0x15u) return r;                      // per stream: 0 = rANS, 1 = RAW; everything else reserved
-    r.raw[LIT] = modes & 1u; r.raw[LEN] = (modes >> 2) & 1u; r.raw[OFF] = (modes >> 4) & 1u;
+    if (modes & 0xC0u) return r;                       // per stream: 0 = rANS, 1 = RAW, 2 = CONST; 3 and bits 6-7 reserved
+    r.raw[LIT] = modes & 3u; r.raw[LEN] = (modes >> 2) & 3u; r.raw[OFF] = (modes >> 4) & 3u;
+    if (r.raw[LIT] == 3u || r.raw[LEN] == 3u || r.raw[OFF] == 3u) return r;
     if (r.n_extras > 2 * r.n_seq) return r;
     r.n_sym[LIT] = r.n_lit;
     r.n_sym[LEN] = 2 * r.n_seq;
@@ -101,8 +102,10 @@ __device__ inline Record open_record(const Container &cv, uint64_t b)
         r.tbl_off[s] = pos;
         if (r.tbl_bytes[s] > 32 + 512) return r;
         pos += r.tbl_bytes[s];
-        if (r.raw[s]) {                                // no table; the symbols sit in the words section
+        if (r.raw[s] == 1u) {                          // RAW: no table; the symbols sit in the words section
             if (r.n_sym[s] == 0 || r.tbl_bytes[s] != 0 || r.n_words[s] != (r.n_sym[s] + 1) / 2) return r;
+        } else if (r.raw[s] == 2u) {                   // CONST: no table; one word whose low byte is the symbol
+            if (r.n_sym[s] == 0 || r.tbl_bytes[s] != 0 || r.n_words[s] != 1) return r;
         } else {
             if ((r.n_sym[s] == 0) != (r.tbl_bytes[s] == 0)) return r;
             if (r.n_words[s] > r.n_sym[s]) return r;

@@ -574,7 +574,9 @@ def test_rejects_inconsistent_raw_streams(binding):
     recs = [build_record(b * B, s, l, raw=("len",)) for b, (s, l) in enumerate(blocks)]
     good = build_container(total, recs)
     i = oracle.info(good)
-    bad = good.copy(); bad[i.payload_off + 7] = 0x08                      # reserved mode 2 for LEN
+    bad = good.copy(); bad[i.payload_off + 7] = 0x0C                      # reserved mode 3 for LEN
+    assert open_rc(binding, bad) == binding.E_CORRUPT
+    bad = good.copy(); bad[i.payload_off + 7] = 0x08                      # CONST for LEN, but its n_words is not 1
     assert open_rc(binding, bad) == binding.E_CORRUPT
     bad = good.copy(); bad[i.payload_off + 8 + 4] ^= 1                    # n_words[LEN] != ceil(n_sym / 2)
     assert open_rc(binding, bad) == binding.E_CORRUPT
@@ -587,6 +589,34 @@ def test_rejects_inconsistent_raw_streams(binding):
     full_check(binding, c, np.frombuffer(b"abc", np.uint8), n_targets=1)
     bad = c.copy(); bad[oracle.info(c).payload_off + 32 + 3] = 1          # pad byte of the odd raw stream
     expect_corrupt(binding, bad, 3, 0)
+
+
+def test_const_streams_handmade_and_encoder_chosen(binding):
+    """CONST stream mode (FORMAT.md section 2 mode 2): containers whose LIT / LEN / OFF streams are constant by
+    construction (tests/test_oracle_codec.py const_case), the encoder's own choice on equal bytes, malformed records."""
+    from test_oracle_codec import const_case
+    total, blocks = const_case()
+    want = np.frombuffer(expand(total, blocks), np.uint8)
+    for const in [("lit",), ("len",), ("off",), ("lit", "len", "off")]:
+        recs = []
+        for b, (seqs, lits) in enumerate(blocks):
+            use = tuple(k for k in const if k == "lit" or seqs)
+            recs.append(build_record(b * B, seqs, lits, const=use))
+        full_check(binding, build_container(total, recs), want, n_targets=2)
+    data = np.frombuffer(ADVERSARIAL["all_equal"], np.uint8)
+    c, st = oracle.encode(data, return_stats=True)
+    assert sum(st.n_const) >= 1
+    full_check(binding, c, data, n_targets=2)
+    # malformed: a state that is not 2^16, a non-zero high byte of the word
+    recs = [build_record(b * B, s, l, const=("lit",)) for b, (s, l) in enumerate(blocks)]
+    good = build_container(total, recs)
+    i = oracle.info(good)
+    bad = good.copy(); bad[64 + (i.n_blocks + 1) * 8 + 5 * 4] ^= 1        # block 0, LIT, lane 5
+    expect_corrupt(binding, bad, total, 0)
+    bad = good.copy(); bad[i.payload_off + 33] = 1                        # block 0: the LIT word sits at record offset 32
+    expect_corrupt(binding, bad, total, 0)
+    bad = good.copy(); bad[i.payload_off + 8] = 2                         # n_words[LIT] != 1
+    assert open_rc(binding, bad) == binding.E_CORRUPT
 
 
 # ------------------------------------------------------------------ seeded fuzz over sizes and encoder policies
